@@ -1,0 +1,223 @@
+"""Pins for the oracle's gridder (orc_grid) and finaliser, and the end-to-end checks.
+
+What fixes them: the definition eq 4.1/4.4 worked with
+Python loops on a RANDOM (asymmetric) injected bank, so a transposed kernel, a
+swapped off_u/off_v or a wrong tap origin fails; the update counts the thesis prints
+(:1572, :1765: 7x7 -> 49, x4 pol -> 196; 29x29 -> 841); the grid-sum identity; the
+conjugate symmetry V(u,v,w) = conj V(-u,-v,-w) (:1418); and the measurement
+equation 1.14 (:399) through a brute-force direct-Fourier image.
+"""
+import numpy as np
+import pytest
+
+C = 299792458.0
+
+
+def _random_bank(rng, supports, beta):
+    supports = np.asarray(supports)
+    off = np.zeros(supports.size, dtype=np.int64)
+    off[1:] = np.cumsum(supports[:-1] ** 2 * beta * beta)
+    total = int((supports ** 2).sum() * beta * beta)
+    return rng.standard_normal(total) + 1j * rng.standard_normal(total), off
+
+
+def test_unit_visibility_reproduces_selected_kernel(orc):
+    rng = np.random.default_rng(11)
+    n, beta, du, P, wmax = 64, 4, 10.0, 3, 100.0
+    sup = np.array([5, 7, 9])
+    bank, off = _random_bank(rng, sup, beta)
+    cases = [(3.30, -2.10, 0.0), (-7.26, 4.51, 30.0), (10.49, 10.74, 100.0), (0.0, 0.0, -100.0), (-20.0, 19.9, 60.0)]
+    for (uc, vc, w) in cases:                      # uc, vc in cells
+        uvw = np.array([[uc * du, vc * du, w]])
+        idx = orc.index_records(uvw, [C], n, 1 / (n * du), beta, P, wmax, sup)
+        vis = np.ones((1, 1, 1), np.complex64)
+        g, nrm, st = orc.grid_records(idx, vis, np.ones((1, 1, 1), np.float32), n, beta, sup, bank, off)
+        # expected, by hand from eq 4.1-4.2: nearest sample, cell, offset (signs flipped if w<0)
+        s = -1.0 if w < 0 else 1.0
+        U = int(np.ceil(s * uc * beta - 0.5)); V = int(np.ceil(s * vc * beta - 0.5))
+        x = (U + 1) // 4; y = (V + 1) // 4           # beta=4: offsets in {-1,0,1,2}
+        ou, ov = U - 4 * x, V - 4 * y
+        p = int(np.floor(np.sqrt(abs(w) / wmax) * (P - 1) + 0.5))
+        S = sup[p]; h = (S - 1) // 2
+        K = bank[off[p]: off[p] + S * S * 16].reshape(4, 4, S, S)[ov + 1, ou + 1]
+        want = np.zeros((n, n), complex)
+        want[y + n // 2 - h: y + n // 2 + h + 1, x + n // 2 - h: x + n // 2 + h + 1] = K
+        assert np.array_equal(g[:, :, 0], want), (uc, vc, w)
+        assert nrm[0] == pytest.approx(K.real.sum(), rel=1e-14)            # eq 4.3 / 4.5
+        assert st.tolist() == [1, 0, S * S]
+
+
+def test_definition_by_python_loops(orc):
+    """Whole eq 4.4 on a few hundred multi-channel, multi-polarised records."""
+    rng = np.random.default_rng(12)
+    n, beta, du, P, wmax, npol = 48, 2, 12.0, 4, 300.0, 2
+    sup = np.array([3, 5, 5, 7])
+    bank, off = _random_bank(rng, sup, beta)
+    nrow, freqs = 150, np.array([C, 1.2 * C])
+    uvw = np.column_stack([rng.uniform(-200, 200, nrow), rng.uniform(-200, 200, nrow), rng.uniform(-250, 250, nrow)])
+    vis = (rng.standard_normal((nrow, 2, npol)) + 1j * rng.standard_normal((nrow, 2, npol))).astype(np.complex64)
+    wt = rng.uniform(0.5, 1, (nrow, 2, npol)).astype(np.float32)
+    wt[3] = 0.0                                            # fully flagged record: dropped (:1315)
+    wt[5, 0, 1] = 0.0                                      # one flagged polarisation: zeros gridded (:1286)
+    idx = orc.index_records(uvw, freqs, n, 1 / (n * du), beta, P, wmax, sup)
+    g, nrm, st = orc.grid_records(idx, vis, wt, n, beta, sup, bank, off)
+    want = np.zeros((n, n, npol), complex)
+    wn = np.zeros(npol)
+    cnt = [0, 0, 0]
+    for r in range(nrow):
+        for c in range(2):
+            lam = freqs[c] / C
+            u, v, w = uvw[r] * lam
+            V = vis[r, c].astype(complex)
+            if w < 0:
+                u, v, w, V = -u, -v, -w, V.conj()
+            U = int(np.ceil(u / du * beta - 0.5)); Vs = int(np.ceil(v / du * beta - 0.5))
+            x, y = U // 2, Vs // 2                         # beta=2: offsets in {0,1}
+            ou, ov = U - 2 * x, Vs - 2 * y
+            p = min(P - 1, int(np.floor(np.sqrt(w / wmax) * (P - 1) + 0.5)))
+            S = sup[p]; h = (S - 1) // 2
+            X, Y = x + n // 2, y + n // 2
+            if X - h < 0 or Y - h < 0 or X + h > n - 1 or Y + h > n - 1 or not wt[r, c].any():
+                cnt[1] += 1
+                continue
+            K = bank[off[p]: off[p] + S * S * 4].reshape(2, 2, S, S)[ov, ou]
+            for ty in range(-h, h + 1):
+                for tx in range(-h, h + 1):
+                    want[Y + ty, X + tx] += wt[r, c].astype(float) * V * K[ty + h, tx + h]
+            wn += wt[r, c] * K.real.sum()
+            cnt[0] += 1
+            cnt[2] += S * S * npol
+    assert cnt[1] > 1
+    assert np.abs(g - want).max() < 1e-12
+    assert np.allclose(nrm, wn, rtol=1e-13)
+    assert st.tolist() == cnt
+    # additive over two calls (thesis feeds chunks, :1011)
+    half = nrow // 2
+    sub = lambda d, a, b: {k: v[a:b] for k, v in d.items()}
+    g2, n2, s2 = orc.grid_records(sub(idx, 0, half), vis[:half], wt[:half], n, beta, sup, bank, off)
+    g2, n2, s2 = orc.grid_records(sub(idx, half, nrow), vis[half:], wt[half:], n, beta, sup, bank, off, g2, n2, s2)
+    assert np.abs(g2 - g).max() < 1e-12 and s2.tolist() == cnt
+
+
+def test_update_counts_printed_in_thesis(orc):
+    """7x7 -> 49 updates per polarisation, x4 = 196 (:1572, :1765); 29x29 = 841 (:1924)."""
+    for S, npol, want in ((7, 1, 49), (7, 4, 196), (29, 1, 841)):
+        bank, off = _random_bank(np.random.default_rng(1), [S], 1)
+        idx = orc.index_records([[0.0, 0.0, 0.0]], [C], 128, 1 / (128 * 10.0), 1, 1, 0.0, [S])
+        _, _, st = orc.grid_records(idx, np.ones((1, 1, npol), np.complex64), np.ones((1, 1, npol), np.float32),
+                                    128, 1, [S], bank, off)
+        assert st.tolist() == [1, 0, want]
+
+
+def _case(rng, nrec, n, du, wmax, frac=0.35):
+    umax = frac * n * du
+    return (rng.uniform(-umax, umax, nrec), rng.uniform(-umax, umax, nrec), rng.uniform(-wmax, wmax, nrec))
+
+
+def test_grid_sum_identity_and_conj_symmetry(orc):
+    from paper_1403_4209_b200 import synth
+    rng = np.random.default_rng(13)
+    n, beta, du, P, wmax, npol = 96, 4, 15.0, 6, 800.0, 4
+    sup = synth.support_table(P, 5, 13)
+    bank, off = orc.build_bank(sup, wmax, du, beta, 13)
+    u, v, w = _case(rng, 400, n, du, wmax)
+    uvw = np.column_stack([u, v, w])
+    vis = (rng.standard_normal((400, 1, npol)) + 1j * rng.standard_normal((400, 1, npol))).astype(np.complex64)
+    wt = rng.uniform(0.5, 1, (400, 1, npol)).astype(np.float32)
+    idx = orc.index_records(uvw, [C], n, 1 / (n * du), beta, P, wmax, sup)
+    g, nrm, st = orc.grid_records(idx, vis, wt, n, beta, sup, bank, off)
+    assert st[1] == 0
+    # sum over cells == sum_i a_i * sum(K_i)
+    tot = np.zeros(npol, complex)
+    for i in range(400):
+        p, S = idx["plane"][i, 0], sup[idx["plane"][i, 0]]
+        K = bank[off[p]: off[p] + S * S * 16].reshape(4, 4, S * S)[idx["off_v"][i, 0] + 1, idx["off_u"][i, 0] + 1]
+        a = wt[i, 0].astype(float) * (vis[i, 0].conj() if w[i] < 0 else vis[i, 0]).astype(complex)
+        tot += a * K.sum()
+    assert np.allclose(g.sum(axis=(0, 1)), tot, rtol=1e-12)
+    # V(u,v,w) and conj V(-u,-v,-w) are the same measurement (:1418): identical grids
+    g2, nrm2, _ = orc.grid_records(orc.index_records(-uvw, [C], n, 1 / (n * du), beta, P, wmax, sup),
+                                   vis.conj(), wt, n, beta, sup, bank, off)
+    assert np.array_equal(g, g2) and np.array_equal(nrm, nrm2)
+
+
+def test_on_sample_case_equals_direct_fourier_exactly(orc):
+    """P=1 and every (u,v) on a grid cell centre (offset 0): the gridded image divided by the exact
+    discrete transform of the S x S taps equals the brute-force direct-Fourier image (eq 1.14) x sum(wt)."""
+    rng = np.random.default_rng(14)
+    n, beta, du, S = 32, 4, 20.0, 7
+    bank, off = orc.build_bank([S], 0.0, du, beta, S)
+    nrec = 60
+    xc = rng.integers(-10, 11, nrec); yc = rng.integers(-10, 11, nrec)
+    u, v = xc * du, yc * du
+    vis = (rng.standard_normal(nrec) + 1j * rng.standard_normal(nrec)).astype(np.complex64)
+    wt = rng.uniform(0.5, 1, nrec).astype(np.float32)
+    uvw = np.column_stack([u, v, np.zeros(nrec)])
+    idx = orc.index_records(uvw, [C], n, 1 / (n * du), beta, 1, 0.0, [S])
+    assert np.all(idx["off_u"] == 0) and np.all(idx["off_v"] == 0)
+    g, nrm, _ = orc.grid_records(idx, vis.reshape(-1, 1, 1), wt.reshape(-1, 1, 1), n, beta, [S], bank, off)
+    img = orc.transform_grid(g)[0]
+    K0 = bank[(1 * beta + 1) * S * S: (1 * beta + 1) * S * S + S * S].reshape(S, S)
+    a = np.arange(-n // 2, n // 2)
+    t = np.arange(-3, 4)
+    E = np.exp(2j * np.pi * np.outer(a, t) / n)
+    chat = E @ K0 @ E.T                                     # [b][a]
+    D = orc.direct_image(u, v, np.zeros(nrec), vis.astype(complex), wt.astype(float), n, du) * wt.astype(float).sum()
+    # direct_image takes the real part; compare real parts of the complex quotient
+    assert np.abs((img / chat).real - D).max() < 1e-11 * np.abs(D).max() * n
+
+
+def test_dirty_image_matches_direct_fourier_within_aliasing(orc):
+    """config-1-like tiny case, no w-term: Alg 4.6 output vs eq 1.14 adjoint on the inner half of
+    the image. The bound (2e-2 of the peak, beta=8, S=7) is DESIGN.md's; the paper gives none
+    ("parity unpinned" for the size of this bound) - but the error must fall as beta grows."""
+    rng = np.random.default_rng(15)
+    n, du, S = 64, 20.0, 7
+    u, v, _ = _case(rng, 300, n, du, 0.0)
+    src = [(9, -5, 1.0), (-12, 14, 0.6)]
+    lm = lambda k: k / (n * du)
+    vis = sum(f * np.exp(-2j * np.pi * (u * lm(a) + v * lm(b))) for a, b, f in src)
+    uvw = np.column_stack([u, v, np.zeros_like(u)])
+    D = orc.direct_image(u, v, np.zeros_like(u), vis, np.ones_like(u), n, du)
+    errs = []
+    for beta in (2, 8):
+        bank, off = orc.build_bank([S], 0.0, du, beta, S)
+        idx = orc.index_records(uvw, [C], n, 1 / (n * du), beta, 1, 0.0, [S])
+        g, nrm, _ = orc.grid_records(idx, vis.astype(np.complex64).reshape(-1, 1, 1), np.ones((300, 1, 1), np.float32),
+                                     n, beta, [S], bank, off)
+        img = orc.finalize(g, nrm, beta)[0]
+        inner = slice(n // 4, 3 * n // 4)
+        errs.append(np.abs(img - D)[inner, inner].max() / np.abs(D).max())
+    assert errs[1] < 2e-2 and errs[1] < errs[0]
+    assert np.unravel_index(np.argmax(img), img.shape) == (-5 + n // 2, 9 + n // 2)
+
+
+def test_w_projection_restores_off_centre_source(orc):
+    """Point source far off-centre with large w: with W-projection the dirty image peaks at the source
+    with ~unit amplitude; with the w-term ignored (P=1) the same data smears. Pins the sign of the
+    w-screen against the measurement equation (eq 1.14 :399, eq 2.14 :580)."""
+    from paper_1403_4209_b200 import synth
+    rng = np.random.default_rng(16)
+    n, du, beta, wmax = 128, 20.0, 8, 6000.0
+    u, v, w = _case(rng, 500, n, du, wmax)
+    a0, b0 = 30, -22
+    l0, m0 = a0 / (n * du), b0 / (n * du)
+    n0 = np.sqrt(1 - l0 * l0 - m0 * m0) - 1
+    assert abs(2 * np.pi * wmax * n0) > 3.0                 # several radians of w-phase
+    vis = np.exp(-2j * np.pi * (u * l0 + v * m0 + w * n0))
+    uvw = np.column_stack([u, v, w])
+    amp = {}
+    for label, P, smax in (("plain", 1, 7), ("wproj", 24, 31)):
+        sup = synth.support_table(P, 7, smax)
+        bank, off = orc.build_bank(sup, wmax, du, beta, smax)
+        idx = orc.index_records(uvw, [C], n, 1 / (n * du), beta, P, wmax, sup)
+        g, nrm, st = orc.grid_records(idx, vis.astype(np.complex64).reshape(-1, 1, 1), np.ones((500, 1, 1), np.float32),
+                                      n, beta, sup, bank, off)
+        img = orc.finalize(g, nrm, beta)[0]
+        amp[label] = img[b0 + n // 2, a0 + n // 2]
+        if label == "wproj":
+            assert np.unravel_index(np.argmax(img), img.shape) == (b0 + n // 2, a0 + n // 2)
+            D = orc.direct_image(u, v, w, vis, np.ones_like(u), n, du)
+            inner = slice(n // 4, 3 * n // 4)
+            assert np.abs(img - D)[inner, inner].max() < 3e-2
+    assert amp["wproj"] > 0.97 and amp["plain"] < 0.6
