@@ -1,0 +1,150 @@
+/* ig.h - C ABI of the B200 convolutional gridder with W-projection.
+ *
+ * The operations are the ones the thesis states (citations are PAPER.md line :
+ * section / equation; "reading k" = DESIGN.md table of readings):
+ *   ig_build_wkernels  Algorithm 4.1 (:1122-1149), bank layout :1100-1108, eq 4.1-4.3
+ *   ig_grid            WImager, eq 4.4a/b and 4.5 (:1266-1293); record preparation
+ *                      sec 4.4.5 (:1385-1444); ordering :714, :1613-1646; plan eq 4.8
+ *   ig_finalize        Algorithm 4.6 (:1664-1676), eq 2.9 (:523), eq 2.13 (:561-564)
+ *   ig_get_stats       eq 4.17 (:1552-1572), metric definitions sec 5.3 (:1757-1779)
+ *
+ * Conventions
+ *  - Plain C, no torch types. Every pointer says host or dev(ice). The caller owns
+ *    ALL buffers and the CUDA stream; the library never allocates or frees device
+ *    memory (PyTorch does, in the Python binding and in the tests).
+ *  - Every call returns an ig_status; nothing throws or aborts across the ABI.
+ *    ig_last_error() gives the text of the last failure on that context.
+ *  - Work is enqueued on the bound stream and calls return without waiting, except
+ *    the calls that hand back host data (ig_finalize's normaliser, ig_get_stats,
+ *    ig_debug_*), which synchronise the stream first.
+ *  - State machine: create -> bind -> build_wkernels (or debug_set_wkernels) ->
+ *    grid* -> finalize. A call out of order returns IG_ESTATE.
+ *  - One context = one grid (thesis: one WImager instance per grid, :1120).
+ *  - There is no CPU fallback anywhere: without a CUDA device every compute call
+ *    returns IG_ECUDA.
+ */
+#ifndef IG_H
+#define IG_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ig_ctx ig_ctx; /* opaque */
+
+typedef enum {
+    IG_OK = 0,
+    IG_EINVAL = 1,      /* bad argument */
+    IG_ESTATE = 2,      /* call out of order */
+    IG_ECUDA = 3,       /* CUDA runtime error (text in ig_last_error) */
+    IG_ENOMEM = 4,      /* a caller-provided buffer is too small */
+    IG_EUNSUPPORTED = 5 /* valid request this build does not implement */
+} ig_status;
+
+#define IG_C_M_S 299792458.0 /* speed of light used for metres -> wavelengths */
+#define IG_MAX_SUPPORT 255   /* record headers carry the support in 8 bits */
+
+/* Create a context. No device work.
+ *   grid_n        grid side N, even, 16..32768
+ *   cell_rad      image pixel size in radians; uv cell du = 1/(N*cell_rad) wavelengths
+ *   n_wplanes     P >= 1 w-planes spaced in sqrt(w) (:633,:1068); 1 = plain gridding
+ *   oversampling  beta in 1..16 (eq 2.11 :548)
+ *   max_support   largest kernel support, odd, 3..IG_MAX_SUPPORT
+ *   n_pol         1, 2 or 4 polarisations (:1025,:1377)                           */
+ig_status ig_create(ig_ctx** out, int grid_n, double cell_rad, int n_wplanes, int oversampling,
+                    int max_support, int n_pol);
+void ig_destroy(ig_ctx* ctx);
+const char* ig_last_error(const ig_ctx* ctx);
+
+/* Bytes of the uv-grid: N*N*n_pol complex64, layout [y][x][pol][re,im]
+ * ("multi-polarised pixel", :1319; reading 13). Pixel (N/2,N/2) is u=v=0. */
+size_t ig_grid_bytes(const ig_ctx* ctx);
+/* Bytes of work_dev that one ig_grid call of (nrow, nchan) needs. */
+size_t ig_workspace_bytes(const ig_ctx* ctx, long long nrow, int nchan);
+/* Bytes of the kernel bank for this support table [n_wplanes] (host; NULL = upper
+ * bound with every plane at max_support). */
+size_t ig_bank_bytes(const ig_ctx* ctx, const int* support_table);
+/* Bytes of work_dev that ig_finalize needs. */
+size_t ig_finalize_workspace_bytes(const ig_ctx* ctx);
+
+/* Bind caller-owned device memory and the stream.
+ *   grid_dev   dev, ig_grid_bytes(); ig_grid ADDS into it, the caller zeroes it
+ *   work_dev   dev, 256-byte aligned scratch, contents undefined between calls
+ *   bank_dev   dev, holds the kernel bank from ig_build_wkernels on; read-only after
+ *   cuda_stream  a cudaStream_t (0 = default stream)
+ * May be called again to change buffers; the bank must then be rebuilt if bank_dev moved. */
+ig_status ig_bind(ig_ctx* ctx, void* grid_dev, size_t grid_bytes, void* work_dev, size_t work_bytes,
+                  void* bank_dev, size_t bank_bytes, void* cuda_stream);
+
+/* Build the bank on the device (Algorithm 4.1 as a direct DFT, reading 5):
+ *   C_p = DFT_{beta*n zero padded}( psi(l) psi(m) exp(+j 2 pi w_p (sqrt(1-l^2-m^2)-1)) ) / A,
+ *   w_p = w_max (p/(P-1))^2, C_0(0,0) = 1, psi = prolate-spheroidal taper (reading 6),
+ *   K[p][ov][ou][ty][tx] = C_p[ty*beta - off_v][tx*beta - off_u], complex64, each S_p x S_p
+ *   matrix contiguous (layout C-1 :1100-1108), plus zeta sums (eq 4.3) kept on the device.
+ *   support_table  host [n_wplanes], odd, 1..max_support. NULL = IG_EUNSUPPORTED for now
+ *                  (auto 1e-3 rule :1114 is "next").
+ * Uses work_dev as scratch. Asynchronous. */
+ig_status ig_build_wkernels(ig_ctx* ctx, double w_max_lambda, const int* support_table);
+
+/* Test hook: install a bank computed elsewhere (the oracle's), same layout, complex64
+ * as float pairs, host memory; zeta sums are recomputed from it. Sets w_max too. */
+ig_status ig_debug_set_wkernels(ig_ctx* ctx, double w_max_lambda, const int* support_table,
+                                const float* bank_host, size_t bank_bytes);
+/* Test hook: copy the device bank to host (complex64 pairs). Synchronises. */
+ig_status ig_debug_get_wkernels(ig_ctx* ctx, float* bank_host, size_t bank_bytes);
+
+/* Grid one batch of visibilities, ADDING into the bound grid (eq 4.4). May be called
+ * many times (the thesis feeds chunks, :1011). Steps, all on the device:
+ *   A2 order rows by baseline (stable, so time stays ascending), records then run
+ *      baseline -> channel -> time;  A1 per record: conj flip for w<0 (eq 4.10), nearest
+ *      oversampled sample, cell, sub-cell offsets, w-plane (readings 2-4), weighted
+ *      visibility (eq 4.16);  A3 records whose footprint leaves the grid or whose weights
+ *      are all zero are dropped (:1278,:1315), the stream is cut into work items;
+ *   C  the gridder.
+ *   uvw_m        dev f64 [nrow][3], metres
+ *   baseline_id  dev i32 [nrow], any non-negative ids; rows in any order
+ *   freqs_hz     HOST f64 [nchan]
+ *   vis          dev f32 [nrow][nchan][n_pol][2]
+ *   weights      dev f32 [nrow][nchan][n_pol]; weight 0 = flagged (:1286)
+ * Asynchronous; inputs must stay valid until the stream reaches the end of the call. */
+ig_status ig_grid(ig_ctx* ctx, const double* uvw_m, const int* baseline_id, long long nrow,
+                  const double* freqs_hz, int nchan, const float* vis, const float* weights);
+
+/* Same, with HOST inputs: copies them to staging areas inside work_dev (which must be
+ * ig_workspace_bytes() + ig_host_staging_bytes() large) and grids. The end-to-end leg. */
+size_t ig_host_staging_bytes(const ig_ctx* ctx, long long nrow, int nchan);
+ig_status ig_grid_host(ig_ctx* ctx, const double* uvw_m, const int* baseline_id, long long nrow,
+                       const double* freqs_hz, int nchan, const float* vis, const float* weights);
+
+/* Algorithm 4.6: inverse FFT per polarisation (uv origin at pixel (N/2,N/2), +j sign,
+ * unnormalised, eq 2.8 :516), real part divided by the normaliser (eq 4.5), the taper
+ * (eq 2.9) and the sinc of the nearest-sample lookup (eq 2.13). No Stokes conversion.
+ *   image_dev        dev f32 [n_pol][N][N], pixel (N/2,N/2) = phase centre
+ *   normaliser_host  HOST f64 [n_pol], receives N_p; may be NULL
+ * Uses work_dev (ig_finalize_workspace_bytes()). Synchronises. */
+ig_status ig_finalize(ig_ctx* ctx, float* image_dev, double* normaliser_host);
+
+/* eq 4.17: records gridded, records dropped, grid-point updates = sum S^2 * n_pol.
+ * Cumulative over ig_grid calls. Synchronises. Any pointer may be NULL. */
+ig_status ig_get_stats(ig_ctx* ctx, long long* n_gridded, long long* n_dropped, long long* n_updates);
+/* Device time split of the LAST ig_grid call in milliseconds (CUDA events recorded on the
+ * bound stream): ingest (A1-A3) and gridder (C). Synchronises. */
+ig_status ig_get_timing(ig_ctx* ctx, float* ingest_ms, float* gridder_ms);
+/* Zero the normaliser and the statistics (for a caller that zeroes the grid to start a new
+ * image with the same bank). Asynchronous. */
+ig_status ig_reset_accumulators(ig_ctx* ctx);
+/* Number of kernels the LAST ig_grid call launched. */
+int ig_last_launches(const ig_ctx* ctx);
+
+/* Test hook: the index tuple of every record in INPUT order, six dev i32 arrays
+ * [nrow][nchan]: X, Y, off_u, off_v, plane, flags (bit0 = conjugated, bit1 = on grid).
+ * Same arithmetic as ig_grid's A1 step. Synchronises. */
+ig_status ig_debug_indices(ig_ctx* ctx, const double* uvw_m, long long nrow, const double* freqs_hz,
+                           int nchan, int* X, int* Y, int* off_u, int* off_v, int* plane, int* flags);
+/* Test hook: the taper psi(eta) the bank builder and the finaliser use, host to host. */
+ig_status ig_debug_taper(const double* eta_host, int n, double* psi_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IG_H */

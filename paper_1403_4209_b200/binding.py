@@ -1,0 +1,227 @@
+"""Thin ctypes binding over the C-ABI library libig.so (include/ig.h).
+
+Argument marshalling only: every step of the path runs in the library's CUDA kernels.
+PyTorch owns device memory and the stream. There is no CPU fallback: `load()` raises if
+the library has not been built, and compute calls raise IgError on any failure.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB = None
+
+STATUS = {0: "IG_OK", 1: "IG_EINVAL", 2: "IG_ESTATE", 3: "IG_ECUDA", 4: "IG_ENOMEM", 5: "IG_EUNSUPPORTED"}
+
+_vp, _sz, _ll, _i, _d = C.c_void_p, C.c_size_t, C.c_longlong, C.c_int, C.c_double
+# name -> (restype, argtypes); mirrors include/ig.h one to one
+SIGNATURES = {
+    "ig_create": (_i, [C.POINTER(_vp), _i, _d, _i, _i, _i, _i]),
+    "ig_destroy": (None, [_vp]),
+    "ig_last_error": (C.c_char_p, [_vp]),
+    "ig_grid_bytes": (_sz, [_vp]),
+    "ig_workspace_bytes": (_sz, [_vp, _ll, _i]),
+    "ig_bank_bytes": (_sz, [_vp, _vp]),
+    "ig_finalize_workspace_bytes": (_sz, [_vp]),
+    "ig_bind": (_i, [_vp, _vp, _sz, _vp, _sz, _vp, _sz, _vp]),
+    "ig_build_wkernels": (_i, [_vp, _d, _vp]),
+    "ig_debug_set_wkernels": (_i, [_vp, _d, _vp, _vp, _sz]),
+    "ig_debug_get_wkernels": (_i, [_vp, _vp, _sz]),
+    "ig_grid": (_i, [_vp, _vp, _vp, _ll, _vp, _i, _vp, _vp]),
+    "ig_host_staging_bytes": (_sz, [_vp, _ll, _i]),
+    "ig_grid_host": (_i, [_vp, _vp, _vp, _ll, _vp, _i, _vp, _vp]),
+    "ig_finalize": (_i, [_vp, _vp, _vp]),
+    "ig_get_stats": (_i, [_vp, C.POINTER(_ll), C.POINTER(_ll), C.POINTER(_ll)]),
+    "ig_get_timing": (_i, [_vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]),
+    "ig_reset_accumulators": (_i, [_vp]),
+    "ig_last_launches": (_i, [_vp]),
+    "ig_debug_indices": (_i, [_vp, _vp, _ll, _vp, _i, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "ig_debug_taper": (_i, [_vp, _i, _vp]),
+}
+
+
+class IgError(RuntimeError):
+    pass
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "libig.so")
+
+
+def load():
+    """Load libig.so. Fails loudly if it is missing (run `python -m paper_1403_4209_b200.build`)."""
+    global _LIB
+    if _LIB is None:
+        path = lib_path()
+        if not os.path.exists(path):
+            raise IgError(f"{path} not built: run __graft_entry__.build() or python paper_1403_4209_b200/build.py; "
+                          "there is no CPU fallback")
+        lib = C.CDLL(path)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(lib, name)
+            fn.restype, fn.argtypes = res, args
+        _LIB = lib
+    return _LIB
+
+
+def _np_ptr(a: np.ndarray):
+    return a.ctypes.data_as(_vp)
+
+
+def taper(eta) -> np.ndarray:
+    """psi(eta) as the library computes it (host code, no GPU needed)."""
+    eta = np.ascontiguousarray(eta, dtype=np.float64)
+    out = np.empty_like(eta)
+    st = load().ig_debug_taper(_np_ptr(eta), eta.size, _np_ptr(out))
+    if st:
+        raise IgError(STATUS.get(st, str(st)))
+    return out
+
+
+class Gridder:
+    """One context = one grid. Device buffers are torch tensors owned by this object."""
+
+    def __init__(self, grid_n, cell_rad, n_wplanes, oversampling, max_support, n_pol, device="cuda:0",
+                 stream=None):
+        import torch
+        self.torch = torch
+        self.lib = load()
+        self.device = torch.device(device)
+        self.grid_n, self.n_pol, self.n_wplanes, self.beta = grid_n, n_pol, n_wplanes, oversampling
+        self.max_support = max_support
+        self.ctx = _vp()
+        st = self.lib.ig_create(C.byref(self.ctx), grid_n, cell_rad, n_wplanes, oversampling, max_support, n_pol)
+        if st:
+            raise IgError(f"ig_create: {STATUS.get(st, st)}")
+        self.stream = stream
+        self.grid = None
+        self.work = None
+        self.bank = None
+        self.supports = None
+
+    # -- plumbing ---------------------------------------------------------------------
+    def _check(self, st, what):
+        if st:
+            msg = self.lib.ig_last_error(self.ctx)
+            raise IgError(f"{what}: {STATUS.get(st, st)}: {msg.decode() if msg else ''}")
+
+    def _stream_ptr(self):
+        s = self.stream if self.stream is not None else self.torch.cuda.current_stream(self.device)
+        return _vp(s.cuda_stream)
+
+    def _bind(self):
+        self._check(self.lib.ig_bind(self.ctx, _vp(self.grid.data_ptr()), self.grid.numel() * 4,
+                                     _vp(self.work.data_ptr()), self.work.numel(),
+                                     _vp(self.bank.data_ptr()), self.bank.numel(), self._stream_ptr()), "ig_bind")
+
+    def allocate(self, supports, work_bytes=0):
+        """Allocate grid (zeroed), bank and a work buffer of at least `work_bytes`."""
+        t = self.torch
+        supports = np.ascontiguousarray(supports, dtype=np.int32)
+        assert supports.size == self.n_wplanes
+        self.supports = supports
+        with t.cuda.device(self.device):
+            self.grid = t.zeros((self.grid_n, self.grid_n, self.n_pol, 2), dtype=t.float32, device=self.device)
+            nb = self.lib.ig_bank_bytes(self.ctx, _np_ptr(supports))
+            self.bank = t.empty(nb, dtype=t.uint8, device=self.device)
+            need = max(int(work_bytes), self.lib.ig_workspace_bytes(self.ctx, 0, 1), 1 << 20)
+            self.work = t.empty(need, dtype=t.uint8, device=self.device)
+        self._bind()
+
+    def ensure_work(self, nbytes):
+        if self.work is None or self.work.numel() < nbytes:
+            self.work = None
+            self.work = self.torch.empty(int(nbytes), dtype=self.torch.uint8, device=self.device)
+            self._bind()
+
+    def workspace_bytes(self, nrow, nchan, host=False):
+        n = self.lib.ig_workspace_bytes(self.ctx, nrow, nchan)
+        if host:
+            n += 256 + self.lib.ig_host_staging_bytes(self.ctx, nrow, nchan)
+        return n
+
+    # -- the calls of include/ig.h ----------------------------------------------------
+    def build_wkernels(self, w_max):
+        self._check(self.lib.ig_build_wkernels(self.ctx, float(w_max), _np_ptr(self.supports)), "ig_build_wkernels")
+
+    def debug_set_wkernels(self, w_max, bank_c64: np.ndarray):
+        b = np.ascontiguousarray(bank_c64, dtype=np.complex64)
+        self._check(self.lib.ig_debug_set_wkernels(self.ctx, float(w_max), _np_ptr(self.supports), _np_ptr(b),
+                                                   b.nbytes), "ig_debug_set_wkernels")
+
+    def debug_get_wkernels(self) -> np.ndarray:
+        n = int((self.supports.astype(np.int64) ** 2).sum()) * self.beta * self.beta
+        out = np.empty(n, dtype=np.complex64)
+        self._check(self.lib.ig_debug_get_wkernels(self.ctx, _np_ptr(out), out.nbytes), "ig_debug_get_wkernels")
+        return out
+
+    def grid_visibilities(self, uvw_m, baseline_id, freqs_hz, vis, weights):
+        """Device tensors: uvw_m f64 [nrow,3], baseline_id i32 [nrow], vis c64/f32 [nrow,nchan,npol(,2)],
+        weights f32 [nrow,nchan,npol]; freqs_hz: host numpy f64."""
+        freqs = np.ascontiguousarray(freqs_hz, dtype=np.float64)
+        nrow, nchan = int(uvw_m.shape[0]), int(freqs.size)
+        self.ensure_work(self.workspace_bytes(nrow, nchan))
+        self._check(self.lib.ig_grid(self.ctx, _vp(uvw_m.data_ptr()), _vp(baseline_id.data_ptr()), nrow,
+                                     _np_ptr(freqs), nchan, _vp(vis.data_ptr()), _vp(weights.data_ptr())), "ig_grid")
+
+    def grid_visibilities_host(self, uvw_m, baseline_id, freqs_hz, vis, weights):
+        """Same with HOST buffers (numpy arrays or pinned CPU torch tensors): the end-to-end call."""
+        freqs = np.ascontiguousarray(freqs_hz, dtype=np.float64)
+        nrow, nchan = int(uvw_m.shape[0]), int(freqs.size)
+        self.ensure_work(self.workspace_bytes(nrow, nchan, host=True))
+        ptr = lambda a: _vp(a.data_ptr()) if hasattr(a, "data_ptr") else _np_ptr(a)
+        self._check(self.lib.ig_grid_host(self.ctx, ptr(uvw_m), ptr(baseline_id), nrow, _np_ptr(freqs), nchan,
+                                          ptr(vis), ptr(weights)), "ig_grid_host")
+
+    def finalize(self):
+        t = self.torch
+        self.ensure_work(self.lib.ig_finalize_workspace_bytes(self.ctx))
+        img = t.empty((self.n_pol, self.grid_n, self.grid_n), dtype=t.float32, device=self.device)
+        norm = np.zeros(self.n_pol, dtype=np.float64)
+        self._check(self.lib.ig_finalize(self.ctx, _vp(img.data_ptr()), _np_ptr(norm)), "ig_finalize")
+        return img, norm
+
+    def stats(self):
+        g, d, u = _ll(), _ll(), _ll()
+        self._check(self.lib.ig_get_stats(self.ctx, C.byref(g), C.byref(d), C.byref(u)), "ig_get_stats")
+        return g.value, d.value, u.value
+
+    def timing(self):
+        a, b = C.c_float(), C.c_float()
+        self._check(self.lib.ig_get_timing(self.ctx, C.byref(a), C.byref(b)), "ig_get_timing")
+        return a.value, b.value
+
+    def reset(self):
+        self.grid.zero_()
+        self._check(self.lib.ig_reset_accumulators(self.ctx), "ig_reset_accumulators")
+
+    def last_launches(self) -> int:
+        return int(self.lib.ig_last_launches(self.ctx))
+
+    def debug_indices(self, uvw_m, freqs_hz):
+        t = self.torch
+        freqs = np.ascontiguousarray(freqs_hz, dtype=np.float64)
+        nrow, nchan = int(uvw_m.shape[0]), int(freqs.size)
+        outs = [t.empty((nrow, nchan), dtype=t.int32, device=self.device) for _ in range(6)]
+        self._check(self.lib.ig_debug_indices(self.ctx, _vp(uvw_m.data_ptr()), nrow, _np_ptr(freqs), nchan,
+                                              *[_vp(o.data_ptr()) for o in outs]), "ig_debug_indices")
+        return dict(zip(("X", "Y", "off_u", "off_v", "plane", "flags"), [o.cpu().numpy() for o in outs]))
+
+    def grid_complex(self) -> np.ndarray:
+        """The grid as complex64 numpy [N][N][npol] (synchronises)."""
+        self.torch.cuda.synchronize(self.device)
+        return self.grid.cpu().numpy().view(np.complex64)[..., 0]
+
+    def close(self):
+        if self.ctx:
+            self.lib.ig_destroy(self.ctx)
+            self.ctx = _vp()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,308 @@
+// ig_api.cu - the C ABI of include/ig.h: argument checks, buffer carving, launch order.
+#include <math.h>
+#include <string.h>
+#include "ig_internal.h"
+
+namespace {
+ig_status fail(ig_ctx* c, ig_status s, const std::string& m) { if (c) c->err = m; return s; }
+
+// layout of bank_dev: [IgAccum][planes P][zeta P*beta^2][K data]
+size_t bank_head_bytes(const ig_ctx* c) {
+    size_t b2 = (size_t)c->prm.beta * c->prm.beta;
+    return ig_align(sizeof(IgAccum)) + ig_align((size_t)c->prm.P * sizeof(IgPlaneEntry)) + ig_align((size_t)c->prm.P * b2 * 8);
+}
+size_t bank_elems_of(const ig_ctx* c, const int* table) {
+    size_t b2 = (size_t)c->prm.beta * c->prm.beta, e = 0;
+    for (int p = 0; p < c->prm.P; ++p) {
+        size_t S = table ? (size_t)table[p] : (size_t)c->max_support;
+        e += S * S * b2;
+    }
+    return e;
+}
+bool table_ok(const ig_ctx* c, const int* t) {
+    for (int p = 0; p < c->prm.P; ++p)
+        if (t[p] < 1 || t[p] > c->max_support || (t[p] & 1) == 0) return false;
+    return true;
+}
+struct GridLayout { size_t freqs, perm, sort, smax, records, total; long long nrb, n_chunks; };
+GridLayout grid_layout(const ig_ctx* c, long long nrow, int nchan) {
+    GridLayout L{};
+    L.nrb = (nrow + IG_CH - 1) / IG_CH;
+    L.n_chunks = L.nrb * nchan;
+    size_t o = 0;
+    L.freqs = o; o += ig_align((size_t)nchan * 8);
+    L.perm = o; o += ig_align((size_t)nrow * 4);
+    L.sort = o; o += ig_align(ig_sort_scratch_bytes(nrow));
+    L.smax = o; o += ig_align((size_t)L.n_chunks * 4);
+    L.records = o; o += ig_align((size_t)L.n_chunks * IG_CH * ig_rec_stride(c->prm.npol));
+    L.total = o;
+    return L;
+}
+// installs the support table: host copies, device plane table; device pointers
+int install_table(ig_ctx* c, const int* table) {
+    const int P = c->prm.P;
+    c->support.assign(table, table + P);
+    c->koff.resize(P);
+    size_t e = 0, b2 = (size_t)c->prm.beta * c->prm.beta;
+    for (int p = 0; p < P; ++p) {
+        if (e >= (1ull << 32)) { c->err = "bank larger than 2^32 complex elements"; return -1; }
+        c->koff[p] = (uint32_t)e;
+        e += (size_t)table[p] * table[p] * b2;
+    }
+    if (e >= (1ull << 32)) { c->err = "bank larger than 2^32 complex elements"; return -1; }
+    c->bank_elems = e;
+    if (bank_head_bytes(c) + e * 8 > c->bank_bytes) { c->err = "bank buffer too small (see ig_bank_bytes)"; return -2; }
+    std::vector<IgPlaneEntry> pe(P);
+    for (int p = 0; p < P; ++p) { pe[p].support = table[p]; pe[p].koff = c->koff[p]; }
+    IG_CUDA_OK(c, cudaMemcpyAsync(c->d_planes, pe.data(), (size_t)P * sizeof(IgPlaneEntry), cudaMemcpyHostToDevice, c->stream));
+    IG_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    return 0;
+}
+}  // namespace
+
+extern "C" {
+
+ig_status ig_create(ig_ctx** out, int grid_n, double cell_rad, int n_wplanes, int oversampling, int max_support,
+                    int n_pol) {
+    if (!out) return IG_EINVAL;
+    *out = nullptr;
+    if (grid_n < 16 || grid_n > 32768 || (grid_n & 1)) return IG_EINVAL;
+    if (!(cell_rad > 0.0) || !isfinite(cell_rad)) return IG_EINVAL;
+    if (n_wplanes < 1 || n_wplanes > (1 << 20)) return IG_EINVAL;
+    if (oversampling < 1 || oversampling > 16) return IG_EINVAL;
+    if (max_support < 3 || max_support > IG_MAX_SUPPORT || (max_support & 1) == 0 || max_support > grid_n) return IG_EINVAL;
+    if (n_pol != 1 && n_pol != 2 && n_pol != 4) return IG_EINVAL;
+    ig_ctx* c = new (std::nothrow) ig_ctx();
+    if (!c) return IG_ENOMEM;
+    c->prm.N = grid_n; c->prm.beta = oversampling; c->prm.P = n_wplanes; c->prm.npol = n_pol;
+    c->prm.shift = (oversampling + 1) / 2 - 1;
+    c->cell_rad = cell_rad;
+    c->du = 1.0 / ((double)grid_n * cell_rad);
+    c->prm.ku = (double)oversampling / (IG_C_M_S * c->du);
+    c->prm.kw = 0.0;
+    c->max_support = max_support;
+    *out = c;
+    return IG_OK;
+}
+
+void ig_destroy(ig_ctx* c) {
+    if (!c) return;
+    for (auto& e : c->ev) if (e) cudaEventDestroy(e);
+    delete c;
+}
+
+const char* ig_last_error(const ig_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+size_t ig_grid_bytes(const ig_ctx* c) { return c ? (size_t)c->prm.N * c->prm.N * c->prm.npol * 8 : 0; }
+size_t ig_workspace_bytes(const ig_ctx* c, long long nrow, int nchan) {
+    if (!c || nrow < 0 || nchan < 1) return 0;
+    size_t a = grid_layout(c, nrow, nchan).total, b = ig_bank_scratch_bytes(c);
+    return a > b ? a : b;
+}
+size_t ig_bank_bytes(const ig_ctx* c, const int* table) {
+    if (!c) return 0;
+    return bank_head_bytes(c) + ig_align(bank_elems_of(c, table) * 8);
+}
+size_t ig_finalize_workspace_bytes(const ig_ctx* c) { return c ? ig_finalize_scratch_bytes(c) : 0; }
+size_t ig_host_staging_bytes(const ig_ctx* c, long long nrow, int nchan) {
+    if (!c || nrow < 0 || nchan < 1) return 0;
+    size_t rec = (size_t)nrow * nchan * c->prm.npol;
+    return ig_align((size_t)nrow * 24) + ig_align((size_t)nrow * 4) + ig_align(rec * 8) + ig_align(rec * 4);
+}
+
+ig_status ig_bind(ig_ctx* c, void* grid_dev, size_t grid_bytes, void* work_dev, size_t work_bytes, void* bank_dev,
+                  size_t bank_bytes, void* cuda_stream) {
+    if (!c) return IG_EINVAL;
+    if (!grid_dev || !work_dev || !bank_dev) return fail(c, IG_EINVAL, "null buffer");
+    if (grid_bytes < ig_grid_bytes(c)) return fail(c, IG_ENOMEM, "grid buffer smaller than ig_grid_bytes()");
+    if (bank_bytes < bank_head_bytes(c)) return fail(c, IG_ENOMEM, "bank buffer too small");
+    if (((uintptr_t)work_dev | (uintptr_t)bank_dev | (uintptr_t)grid_dev) & 255) return fail(c, IG_EINVAL, "buffers must be 256-byte aligned");
+    bool moved = (char*)bank_dev != c->bank_buf;
+    c->grid = (float*)grid_dev; c->grid_bytes = grid_bytes;
+    c->work = (char*)work_dev; c->work_bytes = work_bytes;
+    c->bank_buf = (char*)bank_dev; c->bank_bytes = bank_bytes;
+    c->stream = (cudaStream_t)cuda_stream;
+    char* p = c->bank_buf;
+    c->d_acc = (IgAccum*)p; p += ig_align(sizeof(IgAccum));
+    c->d_planes = (IgPlaneEntry*)p; p += ig_align((size_t)c->prm.P * sizeof(IgPlaneEntry));
+    c->d_zeta = (double*)p; p += ig_align((size_t)c->prm.P * c->prm.beta * c->prm.beta * 8);
+    c->d_bank = (float2*)p;
+    if (moved) {
+        c->have_bank = false;
+        cudaError_t e = cudaMemsetAsync(c->d_acc, 0, sizeof(IgAccum), c->stream);
+        if (e != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_bind: ") + cudaGetErrorString(e));
+    }
+    for (auto& ev : c->ev)
+        if (!ev && cudaEventCreate(&ev) != cudaSuccess) return fail(c, IG_ECUDA, "cudaEventCreate failed");
+    c->bound = true;
+    return IG_OK;
+}
+
+static ig_status set_wmax(ig_ctx* c, double w_max) {
+    if (c->prm.P > 1 && !(w_max > 0.0)) return fail(c, IG_EINVAL, "w_max must be > 0 with more than one w-plane");
+    c->w_max = w_max;
+    double pm1 = (double)(c->prm.P - 1);
+    c->prm.kw = (c->prm.P > 1 && w_max > 0.0) ? (pm1 * pm1) / (IG_C_M_S * w_max) : 0.0;
+    return IG_OK;
+}
+
+ig_status ig_build_wkernels(ig_ctx* c, double w_max, const int* table) {
+    if (!c) return IG_EINVAL;
+    if (!c->bound) return fail(c, IG_ESTATE, "ig_bind first");
+    if (!table) return fail(c, IG_EUNSUPPORTED, "automatic support detection is not implemented; pass a support table");
+    if (!table_ok(c, table)) return fail(c, IG_EINVAL, "supports must be odd and within [1, max_support]");
+    ig_status s = set_wmax(c, w_max);
+    if (s != IG_OK) return s;
+    int r = install_table(c, table);
+    if (r < 0) return r == -2 ? IG_ENOMEM : IG_ECUDA;
+    if (ig_launch_bank(c, c->work, c->work_bytes) < 0) return c->err.find("too small") != std::string::npos ? IG_ENOMEM : IG_ECUDA;
+    c->have_bank = true;
+    return IG_OK;
+}
+
+ig_status ig_debug_set_wkernels(ig_ctx* c, double w_max, const int* table, const float* bank_host, size_t bytes) {
+    if (!c || !table || !bank_host) return IG_EINVAL;
+    if (!c->bound) return fail(c, IG_ESTATE, "ig_bind first");
+    if (!table_ok(c, table)) return fail(c, IG_EINVAL, "supports must be odd and within [1, max_support]");
+    ig_status s = set_wmax(c, w_max);
+    if (s != IG_OK) return s;
+    int r = install_table(c, table);
+    if (r < 0) return r == -2 ? IG_ENOMEM : IG_ECUDA;
+    if (bytes != c->bank_elems * 8) return fail(c, IG_EINVAL, "bank size does not match the support table");
+    if (cudaMemcpyAsync(c->d_bank, bank_host, bytes, cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess)
+        return fail(c, IG_ECUDA, "copying the bank failed");
+    if (ig_launch_zeta(c) < 0) return IG_ECUDA;
+    c->have_bank = true;
+    return IG_OK;
+}
+
+ig_status ig_debug_get_wkernels(ig_ctx* c, float* bank_host, size_t bytes) {
+    if (!c || !bank_host) return IG_EINVAL;
+    if (!c->have_bank) return fail(c, IG_ESTATE, "no bank");
+    if (bytes != c->bank_elems * 8) return fail(c, IG_EINVAL, "bank size mismatch");
+    if (cudaMemcpyAsync(bank_host, c->d_bank, bytes, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess)
+        return fail(c, IG_ECUDA, std::string("reading the bank failed: ") + cudaGetErrorString(cudaGetLastError()));
+    return IG_OK;
+}
+
+ig_status ig_grid(ig_ctx* c, const double* uvw, const int* baseline_id, long long nrow, const double* freqs,
+                  int nchan, const float* vis, const float* wt) {
+    if (!c) return IG_EINVAL;
+    if (!c->bound || !c->have_bank) return fail(c, IG_ESTATE, "ig_bind and ig_build_wkernels first");
+    if (nrow < 0 || nchan < 1 || !freqs) return fail(c, IG_EINVAL, "bad nrow/nchan/freqs");
+    c->launches = 0;
+    c->timed = false;
+    if (nrow == 0) return IG_OK;
+    if (!uvw || !baseline_id || !vis || !wt) return fail(c, IG_EINVAL, "null input");
+    GridLayout L = grid_layout(c, nrow, nchan);
+    if (L.total > c->work_bytes) return fail(c, IG_ENOMEM, "work buffer smaller than ig_workspace_bytes()");
+    double* d_freqs = (double*)(c->work + L.freqs);
+    uint32_t* perm = (uint32_t*)(c->work + L.perm);
+    uint32_t* smax = (uint32_t*)(c->work + L.smax);
+    char* records = c->work + L.records;
+    cudaError_t e = cudaEventRecord(c->ev[0], c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_freqs, freqs, (size_t)nchan * 8, cudaMemcpyHostToDevice, c->stream);
+    if (e != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_grid: ") + cudaGetErrorString(e));
+    int n = ig_launch_sort_rows(c, baseline_id, nrow, perm, c->work + L.sort, ig_sort_scratch_bytes(nrow));
+    if (n < 0) return IG_ECUDA;
+    c->launches += n;
+    n = ig_launch_index(c, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, smax);
+    if (n < 0) return IG_ECUDA;
+    c->launches += n;
+    cudaEventRecord(c->ev[1], c->stream);
+    n = ig_launch_gridder(c, records, smax, L.n_chunks);
+    if (n < 0) return IG_ECUDA;
+    c->launches += n;
+    cudaEventRecord(c->ev[2], c->stream);
+    c->timed = true;
+    return IG_OK;
+}
+
+ig_status ig_grid_host(ig_ctx* c, const double* uvw, const int* baseline_id, long long nrow, const double* freqs,
+                       int nchan, const float* vis, const float* wt) {
+    if (!c) return IG_EINVAL;
+    if (!c->bound) return fail(c, IG_ESTATE, "ig_bind first");
+    if (nrow < 0 || nchan < 1) return fail(c, IG_EINVAL, "bad nrow/nchan");
+    if (nrow == 0) return IG_OK;
+    if (!uvw || !baseline_id || !vis || !wt) return fail(c, IG_EINVAL, "null input");
+    size_t base = ig_align(grid_layout(c, nrow, nchan).total);
+    if (base + ig_host_staging_bytes(c, nrow, nchan) > c->work_bytes) return fail(c, IG_ENOMEM, "work buffer smaller than ig_workspace_bytes() + ig_host_staging_bytes()");
+    size_t rec = (size_t)nrow * nchan * c->prm.npol;
+    char* p = c->work + base;
+    double* d_uvw = (double*)p; p += ig_align((size_t)nrow * 24);
+    int* d_bl = (int*)p; p += ig_align((size_t)nrow * 4);
+    float* d_vis = (float*)p; p += ig_align(rec * 8);
+    float* d_wt = (float*)p;
+    cudaError_t e = cudaMemcpyAsync(d_uvw, uvw, (size_t)nrow * 24, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_bl, baseline_id, (size_t)nrow * 4, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_vis, vis, rec * 8, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_wt, wt, rec * 4, cudaMemcpyHostToDevice, c->stream);
+    if (e != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_grid_host: ") + cudaGetErrorString(e));
+    return ig_grid(c, d_uvw, d_bl, nrow, freqs, nchan, d_vis, d_wt);
+}
+
+ig_status ig_finalize(ig_ctx* c, float* image_dev, double* norm_host) {
+    if (!c || !image_dev) return IG_EINVAL;
+    if (!c->bound || !c->have_bank) return fail(c, IG_ESTATE, "nothing to finalise");
+    int r = ig_run_finalize(c, image_dev, norm_host);
+    if (r == -2) return IG_ENOMEM;
+    return r < 0 ? IG_ECUDA : IG_OK;
+}
+
+ig_status ig_get_stats(ig_ctx* c, long long* g, long long* d, long long* u) {
+    if (!c) return IG_EINVAL;
+    if (!c->bound) return fail(c, IG_ESTATE, "ig_bind first");
+    IgAccum a;
+    if (cudaMemcpyAsync(&a, c->d_acc, sizeof(a), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess)
+        return fail(c, IG_ECUDA, std::string("ig_get_stats: ") + cudaGetErrorString(cudaGetLastError()));
+    if (g) *g = (long long)a.gridded;
+    if (d) *d = (long long)a.dropped;
+    if (u) *u = (long long)a.updates;
+    return IG_OK;
+}
+
+ig_status ig_get_timing(ig_ctx* c, float* ingest_ms, float* gridder_ms) {
+    if (!c) return IG_EINVAL;
+    if (!c->timed) return fail(c, IG_ESTATE, "no timed ig_grid call");
+    if (cudaEventSynchronize(c->ev[2]) != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_get_timing: ") + cudaGetErrorString(cudaGetLastError()));
+    float a = 0, b = 0;
+    cudaEventElapsedTime(&a, c->ev[0], c->ev[1]);
+    cudaEventElapsedTime(&b, c->ev[1], c->ev[2]);
+    if (ingest_ms) *ingest_ms = a;
+    if (gridder_ms) *gridder_ms = b;
+    return IG_OK;
+}
+
+ig_status ig_reset_accumulators(ig_ctx* c) {
+    if (!c) return IG_EINVAL;
+    if (!c->bound) return fail(c, IG_ESTATE, "ig_bind first");
+    if (cudaMemsetAsync(c->d_acc, 0, sizeof(IgAccum), c->stream) != cudaSuccess) return fail(c, IG_ECUDA, "memset failed");
+    return IG_OK;
+}
+
+int ig_last_launches(const ig_ctx* c) { return c ? c->launches : 0; }
+
+ig_status ig_debug_indices(ig_ctx* c, const double* uvw, long long nrow, const double* freqs, int nchan, int* X, int* Y,
+                           int* ou, int* ov, int* pl, int* fl) {
+    if (!c || !uvw || !freqs || nrow < 0 || nchan < 1) return IG_EINVAL;
+    if (!c->bound || !c->have_bank) return fail(c, IG_ESTATE, "ig_bind and a support table first");
+    if ((size_t)nchan * 8 > c->work_bytes) return fail(c, IG_ENOMEM, "work buffer too small");
+    double* d_freqs = (double*)c->work;
+    if (cudaMemcpyAsync(d_freqs, freqs, (size_t)nchan * 8, cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
+        return fail(c, IG_ECUDA, "copying freqs failed");
+    if (ig_launch_debug_index(c, uvw, nrow, d_freqs, nchan, X, Y, ou, ov, pl, fl) < 0) return IG_ECUDA;
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_debug_indices: ") + cudaGetErrorString(e));
+    return IG_OK;
+}
+
+ig_status ig_debug_taper(const double* eta, int n, double* psi) {
+    if (!eta || !psi || n < 0) return IG_EINVAL;
+    ig_taper_eval(eta, n, psi);
+    return IG_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,211 @@
+// ig_ingest.cu - steps A1 (index precompute) and A3 (filter + work items).
+//
+// A1 follows PreProcessUVW (sec 4.4.5): per record the conjugate
+// flag (eq 4.10), the cell and sub-cell offset (eq 4.1-4.2 :1076-1091 on the nearest
+// oversampled sample, eq 2.11-2.13 :546-564), the w-plane (:633,:1068), the Romein
+// position tuple (eq 4.7 :1325-1331: a = X-h, c = -a mod S, d = -(Y-h) mod S) and the
+// kernel pointer z_i; plus the weighted, conjugated visibility (eq 4.16 :1544-1548) and
+// the normaliser / statistics terms (eq 4.5, eq 4.17). All coordinate arithmetic is
+// fp64 with explicitly rounded multiplies (no FMA contraction) so that the integers
+// are bit-identical to an IEEE CPU evaluation of the same formulas (DESIGN.md C.1).
+//
+// A3: the thesis compacts the record stream and builds a plan of equal-support chunks
+// (Alg 4.2-4.3, eq 4.8). Here the layout is data-independent instead: records are written
+// at (row block, channel, row in block), every IG_CH consecutive records are one work
+// item, dropped records stay as 16-byte "skip" headers (S = 0), and the only plan datum
+// is the largest support per item. No scan, no host round trip.
+#include "ig_internal.h"
+
+struct IgIndex { int X, Y, ou, ov, p, S, on; };
+
+__device__ __forceinline__ long long floordiv_ll(long long a, long long b) {
+    long long q = a / b;
+    if ((a % b != 0) && ((a < 0) != (b < 0))) q -= 1;
+    return q;
+}
+
+// um, vm, wm already flipped so that wm >= 0
+__device__ __forceinline__ IgIndex ig_index_one(const IgParams& P, const IgPlaneEntry* __restrict__ planes,
+                                                double um, double vm, double wm, double nu) {
+    IgIndex r;
+    double fu = __dmul_rn(__dmul_rn(um, nu), P.ku);
+    double fv = __dmul_rn(__dmul_rn(vm, nu), P.ku);
+    long long U = (long long)ceil(__dsub_rn(fu, 0.5));   // nearest sample, ties towards -inf
+    long long V = (long long)ceil(__dsub_rn(fv, 0.5));
+    long long x = floordiv_ll(U + P.shift, P.beta);      // -du/2 < delta <= du/2 (eq 4.2)
+    long long y = floordiv_ll(V + P.shift, P.beta);
+    r.ou = (int)(U - x * P.beta);
+    r.ov = (int)(V - y * P.beta);
+    int p = 0;
+    if (P.P > 1) {
+        double sp = floor(__dadd_rn(__dsqrt_rn(__dmul_rn(__dmul_rn(wm, nu), P.kw)), 0.5));
+        p = sp >= (double)(P.P - 1) ? P.P - 1 : (int)sp;
+    }
+    r.p = p;
+    r.S = planes[p].support;
+    long long h = (r.S - 1) / 2;
+    long long Xc = x + P.N / 2, Yc = y + P.N / 2;
+    r.on = (Xc - h >= 0) && (Xc + h <= P.N - 1) && (Yc - h >= 0) && (Yc + h <= P.N - 1);
+    const long long lim = 1ll << 30;
+    Xc = Xc < -lim ? -lim : (Xc > lim ? lim : Xc);
+    Yc = Yc < -lim ? -lim : (Yc > lim ? lim : Yc);
+    r.X = (int)Xc; r.Y = (int)Yc;
+    return r;
+}
+
+// One CTA = one row block of IG_CH sorted rows; thread t = row rb*IG_CH + t; loop over channels.
+// Record at place ((rb*nchan + c)*IG_CH + t): 16-byte header {pix_base, kbase, c|d<<8|S<<16|conj<<24, plane}
+// followed by npol complex32 pairs (stride 48 B for 4 pol, else 32 B).
+template <int NPOL>
+__global__ void __launch_bounds__(IG_CH)
+k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __restrict__ zeta,
+        const double* __restrict__ uvw, const uint32_t* __restrict__ perm, long long nrow,
+        const double* __restrict__ freqs, int nchan, const float* __restrict__ vis,
+        const float* __restrict__ wt, char* __restrict__ records, uint32_t* __restrict__ chunk_smax,
+        IgAccum* __restrict__ acc) {
+    constexpr int STRIDE = NPOL == 4 ? 48 : 32;
+    const long long rb = blockIdx.x;
+    const int t = threadIdx.x, lane = t & 31;
+    const long long j = rb * IG_CH + t;
+    const bool live = j < nrow;
+    long long row = 0;
+    double um = 0, vm = 0, wm = 0;
+    int conj = 0;
+    if (live) {
+        row = perm[j];
+        um = uvw[3 * row]; vm = uvw[3 * row + 1]; wm = uvw[3 * row + 2];
+        conj = wm < 0.0;
+        if (conj) { um = -um; vm = -vm; wm = -wm; }
+    }
+    double nsum[NPOL];
+#pragma unroll
+    for (int q = 0; q < NPOL; ++q) nsum[q] = 0.0;
+    unsigned long long n_grid = 0, n_drop = 0, n_upd = 0;
+
+    for (int c = 0; c < nchan; ++c) {
+        const long long chunk = rb * nchan + c;
+        char* rec = records + ((size_t)chunk * IG_CH + t) * STRIDE;
+        uint4 hdr = make_uint4(0u, 0u, 0u, 0u);
+        float v[2 * NPOL];
+#pragma unroll
+        for (int q = 0; q < 2 * NPOL; ++q) v[q] = 0.f;
+        int S = 0;
+        if (live) {
+            IgIndex ix = ig_index_one(P, planes, um, vm, wm, freqs[c]);
+            const float* vp = vis + ((size_t)row * nchan + c) * (2 * NPOL);
+            const float* wp = wt + ((size_t)row * nchan + c) * NPOL;
+            float w[NPOL];
+            bool any = false;
+            if constexpr (NPOL == 4) {
+                float4 w4 = *reinterpret_cast<const float4*>(wp);
+                w[0] = w4.x; w[1] = w4.y; w[2] = w4.z; w[3] = w4.w;
+                float4 a = *reinterpret_cast<const float4*>(vp), b = *reinterpret_cast<const float4*>(vp + 4);
+                v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+            } else {
+#pragma unroll
+                for (int q = 0; q < NPOL; ++q) { w[q] = wp[q]; v[2 * q] = vp[2 * q]; v[2 * q + 1] = vp[2 * q + 1]; }
+            }
+#pragma unroll
+            for (int q = 0; q < NPOL; ++q) any |= (w[q] != 0.f);
+            if (ix.on && any) {
+                S = ix.S;
+                const int h = (S - 1) / 2;
+                const int a0 = ix.X - h, b0 = ix.Y - h;
+                int cm = (-a0) % S; if (cm < 0) cm += S;
+                int dm = (-b0) % S; if (dm < 0) dm += S;
+                const uint32_t tab = (uint32_t)((ix.ov + P.shift) * P.beta + (ix.ou + P.shift));
+                hdr.x = (uint32_t)(b0 * P.N + a0);
+                hdr.y = planes[ix.p].koff + tab * (uint32_t)(S * S);
+                hdr.z = (uint32_t)cm | ((uint32_t)dm << 8) | ((uint32_t)S << 16) | ((uint32_t)conj << 24);
+                hdr.w = (uint32_t)ix.p;
+                const double z = zeta[(size_t)ix.p * P.beta * P.beta + tab];
+#pragma unroll
+                for (int q = 0; q < NPOL; ++q) {
+                    nsum[q] += (double)w[q] * z;              // eq 4.5
+                    v[2 * q] = w[q] * v[2 * q];               // eq 4.16
+                    v[2 * q + 1] = conj ? -(w[q] * v[2 * q + 1]) : w[q] * v[2 * q + 1];
+                }
+                n_grid += 1;
+                n_upd += (unsigned long long)(S * S * NPOL);
+            } else {
+                n_drop += 1;
+            }
+        }
+        *reinterpret_cast<uint4*>(rec) = hdr;
+        if constexpr (NPOL == 4) {
+            *reinterpret_cast<float4*>(rec + 16) = make_float4(v[0], v[1], v[2], v[3]);
+            *reinterpret_cast<float4*>(rec + 32) = make_float4(v[4], v[5], v[6], v[7]);
+        } else if constexpr (NPOL == 2) {
+            *reinterpret_cast<float4*>(rec + 16) = make_float4(v[0], v[1], v[2], v[3]);
+        } else {
+            *reinterpret_cast<float4*>(rec + 16) = make_float4(v[0], v[1], 0.f, 0.f);
+        }
+        unsigned smax = __reduce_max_sync(0xffffffffu, (unsigned)S);
+        if (lane == 0 && smax) atomicMax(&chunk_smax[chunk], smax);
+    }
+
+    // block reduction of the normaliser and the counters
+    __shared__ double sh[IG_CH / 32][NPOL + 3];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int q = 0; q < NPOL; ++q) nsum[q] += __shfl_xor_sync(0xffffffffu, nsum[q], o);
+        n_grid += __shfl_xor_sync(0xffffffffu, n_grid, o);
+        n_drop += __shfl_xor_sync(0xffffffffu, n_drop, o);
+        n_upd += __shfl_xor_sync(0xffffffffu, n_upd, o);
+    }
+    if (lane == 0) {
+#pragma unroll
+        for (int q = 0; q < NPOL; ++q) sh[t >> 5][q] = nsum[q];
+        sh[t >> 5][NPOL] = (double)n_grid; sh[t >> 5][NPOL + 1] = (double)n_drop; sh[t >> 5][NPOL + 2] = (double)n_upd;
+    }
+    __syncthreads();
+    if (t < NPOL + 3) {
+        double s = 0;
+        for (int w = 0; w < IG_CH / 32; ++w) s += sh[w][t];   // counts < 2^53: exact in fp64
+        if (t < NPOL) atomicAdd(&acc->norm[t], s);
+        else if (t == NPOL) atomicAdd(&acc->gridded, (unsigned long long)s);
+        else if (t == NPOL + 1) atomicAdd(&acc->dropped, (unsigned long long)s);
+        else atomicAdd(&acc->updates, (unsigned long long)s);
+    }
+}
+
+__global__ void k_debug_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __restrict__ uvw,
+                              long long nrow, const double* __restrict__ freqs, int nchan, int* X, int* Y, int* ou,
+                              int* ov, int* pl, int* fl) {
+    long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nrow * nchan) return;
+    long long r = k / nchan;
+    int c = (int)(k - r * nchan);
+    double um = uvw[3 * r], vm = uvw[3 * r + 1], wm = uvw[3 * r + 2];
+    int conj = wm < 0.0;
+    if (conj) { um = -um; vm = -vm; wm = -wm; }
+    IgIndex ix = ig_index_one(P, planes, um, vm, wm, freqs[c]);
+    X[k] = ix.X; Y[k] = ix.Y; ou[k] = ix.ou; ov[k] = ix.ov; pl[k] = ix.p; fl[k] = conj | (ix.on << 1);
+}
+
+int ig_launch_index(ig_ctx* c, const double* uvw, const uint32_t* perm, long long nrow, const double* d_freqs,
+                    int nchan, const float* vis, const float* wt, char* records, uint32_t* chunk_smax) {
+    long long nrb = (nrow + IG_CH - 1) / IG_CH;
+    if (nrb == 0) return 0;
+    if (nrb > 0x7fffffffll) { c->err = "too many rows"; return -1; }
+    IG_CUDA_OK(c, cudaMemsetAsync(chunk_smax, 0, (size_t)nrb * nchan * 4, c->stream));
+    dim3 g((unsigned)nrb), b(IG_CH);
+    switch (c->prm.npol) {
+        case 1: k_index<1><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc); break;
+        case 2: k_index<2><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc); break;
+        default: k_index<4><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc); break;
+    }
+    IG_CUDA_OK(c, cudaGetLastError());
+    return 1;
+}
+
+int ig_launch_debug_index(ig_ctx* c, const double* uvw, long long nrow, const double* d_freqs, int nchan, int* X,
+                          int* Y, int* ou, int* ov, int* pl, int* fl) {
+    long long n = nrow * nchan;
+    if (n == 0) return 0;
+    k_debug_index<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->prm, c->d_planes, uvw, nrow, d_freqs, nchan,
+                                                                      X, Y, ou, ov, pl, fl);
+    IG_CUDA_OK(c, cudaGetLastError());
+    return 1;
+}

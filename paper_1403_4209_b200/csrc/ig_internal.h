@@ -1,0 +1,83 @@
+// ig_internal.h - shared declarations of the CUDA path (never included by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+#include "../../include/ig.h"
+
+#define IG_CH 128            // records per chunk (one work item per (row block, channel))
+#define IG_STAGE 32          // records per TMA stage
+#define IG_NSTAGE (IG_CH / IG_STAGE)
+#define IG_RMAX 8            // grid points per lane, at most
+#define IG_GRID_WARPS 4      // warps per gridder CTA
+
+// Device-side tail of the bank buffer: small tables and accumulators.
+struct IgPlaneEntry { int support; uint32_t koff; };   // koff in complex elements
+struct IgAccum {
+    double norm[4];                     // eq 4.5 normaliser per polarisation
+    unsigned long long gridded, dropped, updates;   // eq 4.17
+    unsigned int ticket;                // work queue of the gridder
+    unsigned int max_key;               // largest baseline id of the current call
+};
+
+struct IgParams {            // passed by value to kernels
+    int N, beta, P, npol;
+    int shift;               // ceil(beta/2) - 1
+    double ku, kw;           // index constants (include/ig.h, DESIGN.md C.1)
+};
+
+struct ig_ctx {
+    IgParams prm{};
+    double cell_rad = 0, du = 0, w_max = 0;
+    int max_support = 0;
+    // bound buffers
+    float* grid = nullptr; size_t grid_bytes = 0;
+    char* work = nullptr; size_t work_bytes = 0;
+    char* bank_buf = nullptr; size_t bank_bytes = 0;
+    cudaStream_t stream = nullptr;
+    bool bound = false, have_bank = false;
+    // bank description (host copies)
+    std::vector<int> support;
+    std::vector<uint32_t> koff;
+    size_t bank_elems = 0;
+    // device pointers inside bank_buf
+    float2* d_bank = nullptr; double* d_zeta = nullptr; IgPlaneEntry* d_planes = nullptr;
+    IgAccum* d_acc = nullptr;
+    // timing of the last ig_grid
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    bool timed = false;
+    int launches = 0;
+    std::string err;
+};
+
+static inline size_t ig_align(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+static inline int ig_rec_stride(int npol) { return npol == 4 ? 48 : 32; }  // bytes, multiple of 16
+
+// ig_taper.cpp-ish (host, in ig_bank.cu)
+void ig_taper_eval(const double* eta, int n, double* psi);
+
+// launchers (each returns the number of kernels launched, or -1 with ctx->err set)
+int ig_launch_sort_rows(ig_ctx* c, const int* baseline_id, long long nrow, uint32_t* perm_out,
+                        char* scratch, size_t scratch_bytes);
+size_t ig_sort_scratch_bytes(long long nrow);
+int ig_launch_index(ig_ctx* c, const double* uvw, const uint32_t* perm, long long nrow,
+                    const double* d_freqs, int nchan, const float* vis, const float* wt,
+                    char* records, uint32_t* chunk_smax);
+int ig_launch_debug_index(ig_ctx* c, const double* uvw, long long nrow, const double* d_freqs, int nchan,
+                          int* X, int* Y, int* ou, int* ov, int* pl, int* fl);
+int ig_launch_gridder(ig_ctx* c, const char* records, const uint32_t* chunk_smax, long long n_chunks);
+int ig_launch_bank(ig_ctx* c, char* scratch, size_t scratch_bytes);
+size_t ig_bank_scratch_bytes(const ig_ctx* c);
+int ig_launch_zeta(ig_ctx* c);
+int ig_run_finalize(ig_ctx* c, float* image, double* norm_host);
+size_t ig_finalize_scratch_bytes(const ig_ctx* c);
+
+#define IG_CUDA_OK(ctx, call)                                                        \
+    do {                                                                             \
+        cudaError_t e_ = (call);                                                     \
+        if (e_ != cudaSuccess) {                                                     \
+            (ctx)->err = std::string(#call) + ": " + cudaGetErrorString(e_);         \
+            return -1;                                                               \
+        }                                                                            \
+    } while (0)

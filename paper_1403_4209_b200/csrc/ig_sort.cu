@@ -1,0 +1,159 @@
+// ig_sort.cu - step A2 (ordering): stable LSD radix sort of rows by baseline id.
+//
+// The thesis groups records by baseline with time ascending on the CPU (Alg 4.5,
+// PAPER.md:1613-1646) because the gridder accumulates along a baseline's track (:714).
+// Here the rows (nrow <= a few 1e7; records = rows x channels are never moved by the
+// sort) are ordered on the device: 4 passes of an 8-bit stable counting sort,
+// each = per-tile histogram -> exclusive scan -> stable scatter. Stability keeps the
+// input (time) order inside a baseline. Output: perm[j] = input row at sorted place j.
+#include "ig_internal.h"
+
+#define SORT_THREADS 256
+#define SORT_WARPS (SORT_THREADS / 32)
+#define SORT_STEPS 32
+#define SORT_TILE (SORT_THREADS * SORT_STEPS)   // 8192 keys per CTA
+
+__device__ __forceinline__ uint32_t lanemask_lt() {
+    uint32_t m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+
+// per-warp digit counts of this CTA's tile into smem cnt[warp][256]
+__device__ __forceinline__ void tile_count(const uint32_t* __restrict__ keys, long long n, int shift,
+                                           uint32_t (*cnt)[256]) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int i = threadIdx.x; i < SORT_WARPS * 256; i += SORT_THREADS) (&cnt[0][0])[i] = 0;
+    __syncthreads();
+    const long long base = (long long)blockIdx.x * SORT_TILE + (long long)warp * (32 * SORT_STEPS);
+#pragma unroll 4
+    for (int s = 0; s < SORT_STEPS; ++s) {
+        long long k = base + s * 32 + lane;
+        if (k < n) atomicAdd(&cnt[warp][(keys[k] >> shift) & 255u], 1u);
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(SORT_THREADS)
+k_sort_hist(const uint32_t* __restrict__ keys, long long n, int shift, uint32_t* __restrict__ hist, int nblk) {
+    __shared__ uint32_t cnt[SORT_WARPS][256];
+    tile_count(keys, n, shift, cnt);
+    uint32_t t = 0;
+#pragma unroll
+    for (int w = 0; w < SORT_WARPS; ++w) t += cnt[w][threadIdx.x];
+    hist[(size_t)threadIdx.x * nblk + blockIdx.x] = t;   // bin-major: a flat scan gives global offsets
+}
+
+// in-place exclusive scan of m uint32 values, one CTA of 1024 threads
+__global__ void __launch_bounds__(1024) k_scan_excl(uint32_t* __restrict__ a, long long m) {
+    __shared__ uint32_t wsum[32];
+    __shared__ uint32_t carry_s;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (long long t0 = 0; t0 < m; t0 += 4096) {
+        long long i = t0 + (long long)threadIdx.x * 4;
+        uint32_t v[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) v[k] = (i + k < m) ? a[i + k] : 0u;
+        uint32_t s = v[0] + v[1] + v[2] + v[3], inc = s;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t y = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += y;
+        }
+        if (lane == 31) wsum[warp] = inc;
+        __syncthreads();
+        if (warp == 0) {
+            uint32_t w = wsum[lane], wi = w;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                uint32_t y = __shfl_up_sync(0xffffffffu, wi, o);
+                if (lane >= o) wi += y;
+            }
+            wsum[lane] = wi - w;   // exclusive over warps
+        }
+        __syncthreads();
+        uint32_t carry = carry_s;
+        uint32_t ex = carry + wsum[warp] + (inc - s);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (i + k < m) a[i + k] = ex;
+            ex += v[k];
+        }
+        __syncthreads();
+        if (threadIdx.x == 1023) carry_s = carry + wsum[31] + inc;
+        __syncthreads();
+    }
+}
+
+// vals_in == nullptr means the identity permutation (first pass)
+__global__ void __launch_bounds__(SORT_THREADS)
+k_sort_scatter(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals_in, long long n, int shift,
+               const uint32_t* __restrict__ hist, int nblk, uint32_t* __restrict__ keys_out,
+               uint32_t* __restrict__ vals_out) {
+    __shared__ uint32_t cnt[SORT_WARPS][256];
+    tile_count(keys, n, shift, cnt);
+    {   // turn per-warp counts into per-warp start positions in the output
+        uint32_t run = hist[(size_t)threadIdx.x * nblk + blockIdx.x];
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; ++w) {
+            uint32_t c = cnt[w][threadIdx.x];
+            cnt[w][threadIdx.x] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long base = (long long)blockIdx.x * SORT_TILE + (long long)warp * (32 * SORT_STEPS);
+    for (int s = 0; s < SORT_STEPS; ++s) {
+        long long k = base + s * 32 + lane;
+        bool act = k < n;
+        uint32_t key = act ? keys[k] : 0u;
+        uint32_t d = act ? ((key >> shift) & 255u) : 256u;
+        uint32_t peers = __match_any_sync(0xffffffffu, d);
+        uint32_t b = act ? cnt[warp][d] : 0u;
+        __syncwarp();
+        if (act && (peers & lanemask_lt()) == 0) cnt[warp][d] = b + __popc(peers);
+        __syncwarp();
+        if (act) {
+            uint32_t pos = b + __popc(peers & lanemask_lt());
+            keys_out[pos] = key;
+            vals_out[pos] = vals_in ? vals_in[k] : (uint32_t)k;
+        }
+    }
+}
+
+size_t ig_sort_scratch_bytes(long long nrow) {
+    long long nblk = (nrow + SORT_TILE - 1) / SORT_TILE;
+    if (nblk < 1) nblk = 1;
+    // keysA, keysB, valsB (valsA is the caller's perm_out), hist
+    return 3 * ig_align((size_t)nrow * 4) + ig_align((size_t)nblk * 256 * 4);
+}
+
+int ig_launch_sort_rows(ig_ctx* c, const int* baseline_id, long long nrow, uint32_t* perm_out, char* scratch,
+                        size_t scratch_bytes) {
+    if (nrow >= (1ll << 32)) { c->err = "nrow must be < 2^32"; return -1; }
+    if (scratch_bytes < ig_sort_scratch_bytes(nrow)) { c->err = "sort scratch too small"; return -1; }
+    int nblk = (int)((nrow + SORT_TILE - 1) / SORT_TILE);
+    if (nblk < 1) nblk = 1;
+    size_t a = ig_align((size_t)nrow * 4);
+    uint32_t* keysA = (uint32_t*)scratch;
+    uint32_t* keysB = (uint32_t*)(scratch + a);
+    uint32_t* valsB = (uint32_t*)(scratch + 2 * a);
+    uint32_t* hist = (uint32_t*)(scratch + 3 * a);
+    uint32_t* valsA = perm_out;
+    int launches = 0;
+    for (int pass = 0; pass < 4; ++pass) {
+        const uint32_t* kin = pass == 0 ? (const uint32_t*)baseline_id : ((pass & 1) ? keysB : keysA);
+        const uint32_t* vin = pass == 0 ? nullptr : ((pass & 1) ? valsB : valsA);
+        uint32_t* kout = (pass & 1) ? keysA : keysB;
+        uint32_t* vout = (pass & 1) ? valsA : valsB;
+        k_sort_hist<<<nblk, SORT_THREADS, 0, c->stream>>>(kin, nrow, pass * 8, hist, nblk);
+        k_scan_excl<<<1, 1024, 0, c->stream>>>(hist, (long long)nblk * 256);
+        k_sort_scatter<<<nblk, SORT_THREADS, 0, c->stream>>>(kin, vin, nrow, pass * 8, hist, nblk, kout, vout);
+        launches += 3;
+    }
+    IG_CUDA_OK(c, cudaGetLastError());
+    return launches;   // result is in valsA == perm_out after the 4th pass
+}

@@ -1,0 +1,231 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element.
+
+Bars (BASELINE.json north_star): indices bit-exact; grid relative Frobenius error <= 1e-5 and
+max per-cell |delta| <= 1e-4 * max|grid| for fp32 accumulation against the fp64 oracle.
+Inputs are the seeded synthetic workloads of paper_1403_4209_b200.synth (data only).
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+
+from paper_1403_4209_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+FROB_TOL = 1e-5
+MAX_TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test needs a CUDA device; there is no CPU fallback")
+    return torch
+
+
+def small(cfg, **kw):
+    return dataclasses.replace(cfg, **kw)
+
+
+# reduced versions of the five configurations: same geometry, fewer stations / time steps / planes,
+# sized so that the oracle finishes in seconds while the work still spans many work items
+CASES = {
+    "cfg1": synth.CONFIGS[0],
+    "cfg2s": small(synth.CONFIGS[1], n_station=14, n_time=200),
+    "cfg3s": small(synth.CONFIGS[2], grid_n=1024, n_station=10, n_time=300, n_chan=8, n_wplanes=24),
+    "cfg4s": small(synth.CONFIGS[3], grid_n=2048, n_station=8, n_time=130, n_chan=6, n_wplanes=20),
+    "cfg5s": small(synth.CONFIGS[4], grid_n=2048, n_station=9, n_time=128, n_chan=5, n_wplanes=16, s_max=129),
+    "pol2": small(synth.CONFIGS[1], n_pol=2, n_station=9, n_time=77, n_chan=3, n_wplanes=8),
+}
+
+
+def to_dev(torch, wl):
+    d = "cuda:0"
+    return (torch.from_numpy(wl["uvw_m"]).to(d), torch.from_numpy(wl["baseline"]).to(d),
+            torch.from_numpy(np.ascontiguousarray(wl["vis"])).to(d), torch.from_numpy(wl["weights"]).to(d))
+
+
+def make_gridder(wl):
+    from paper_1403_4209_b200.binding import Gridder
+    cfg = wl["cfg"]
+    g = Gridder(cfg.grid_n, wl["cell_rad"], cfg.n_wplanes, cfg.oversampling, int(wl["supports"].max()), cfg.n_pol)
+    g.allocate(wl["supports"])
+    return g
+
+
+def oracle_run(orc, wl, bank=None, bank_off=None):
+    cfg = wl["cfg"]
+    sup = wl["supports"]
+    if bank is None:
+        bank, bank_off = orc.build_bank(sup, wl["w_max"], wl["du"], cfg.oversampling, int(sup.max()))
+    idx = orc.index_records(wl["uvw_m"], wl["freqs_hz"], cfg.grid_n, wl["cell_rad"], cfg.oversampling,
+                            cfg.n_wplanes, wl["w_max"], sup)
+    grid, norm, stats = orc.grid_records(idx, wl["vis"], wl["weights"], cfg.grid_n, cfg.oversampling, sup, bank, bank_off)
+    return dict(bank=bank, bank_off=bank_off, idx=idx, grid=grid, norm=norm, stats=stats)
+
+
+def check_grid(got, want):
+    want = want.astype(np.complex128)
+    diff = got.astype(np.complex128) - want
+    frob = np.linalg.norm(diff.ravel()) / np.linalg.norm(want.ravel())
+    mx = np.abs(diff).max() / np.abs(want).max()
+    assert frob <= FROB_TOL, f"relative Frobenius error {frob:.3e}"
+    assert mx <= MAX_TOL, f"max |delta| / max|grid| = {mx:.3e}"
+    return frob, mx
+
+
+@pytest.fixture(scope="module")
+def runs(orc, torch_cuda):
+    cache = {}
+
+    def get(name):
+        if name not in cache:
+            wl = synth.make_workload(CASES[name])
+            cache[name] = (wl, oracle_run(orc, wl))
+        return cache[name]
+    return get
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_indices_bit_exact(name, runs, torch_cuda):
+    wl, ref = runs(name)
+    g = make_gridder(wl)
+    g.debug_set_wkernels(wl["w_max"], ref["bank"].astype(np.complex64))
+    uvw = torch_cuda.from_numpy(wl["uvw_m"]).cuda()
+    got = g.debug_indices(uvw, wl["freqs_hz"])
+    for k in ("X", "Y", "off_u", "off_v", "plane", "flags"):
+        assert np.array_equal(got[k], ref["idx"][k]), k
+
+
+@pytest.mark.parametrize("idx", [1, 2, 3, 4])
+def test_indices_bit_exact_full_size_sample(idx, orc, torch_cuda):
+    """Full-size configuration parameters (grid, cell, planes, supports), every k-th row."""
+    cfg = synth.CONFIGS[idx]
+    wl = synth.make_workload(cfg, with_vis=False)
+    step = max(1, wl["uvw_m"].shape[0] // 150_000)
+    uvw = np.ascontiguousarray(wl["uvw_m"][::step])
+    ref = orc.index_records(uvw, wl["freqs_hz"], cfg.grid_n, wl["cell_rad"], cfg.oversampling, cfg.n_wplanes,
+                            wl["w_max"], wl["supports"])
+    from paper_1403_4209_b200.binding import Gridder
+    g = Gridder(cfg.grid_n, wl["cell_rad"], cfg.n_wplanes, cfg.oversampling, int(wl["supports"].max()), 1)
+    g.allocate(wl["supports"])
+    g.debug_set_wkernels(wl["w_max"], np.zeros(int((wl["supports"].astype(np.int64) ** 2).sum()) * cfg.oversampling ** 2,
+                                               dtype=np.complex64))
+    got = g.debug_indices(torch_cuda.from_numpy(uvw).cuda(), wl["freqs_hz"])
+    for k in ("X", "Y", "off_u", "off_v", "plane", "flags"):
+        assert np.array_equal(got[k], ref[k]), k
+    assert (ref["flags"] & 2).all()   # the cell rule keeps every footprint on the grid
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2s", "cfg4s"])
+def test_bank_matches_oracle(name, runs):
+    wl, ref = runs(name)
+    g = make_gridder(wl)
+    g.build_wkernels(wl["w_max"])
+    got = g.debug_get_wkernels()
+    want = ref["bank"]
+    err = np.abs(got.astype(np.complex128) - want).max()
+    assert err <= 2e-7 * np.abs(want).max(), err      # fp64 DFT rounded to fp32: half an ulp of the peak value 1
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_grid_matches_oracle_own_bank(name, runs, torch_cuda):
+    wl, ref = runs(name)
+    g = make_gridder(wl)
+    g.build_wkernels(wl["w_max"])
+    uvw, bl, vis, wt = to_dev(torch_cuda, wl)
+    g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+    check_grid(g.grid_complex(), ref["grid"])
+    gridded, dropped, updates = g.stats()
+    assert (gridded, dropped, updates) == tuple(int(x) for x in ref["stats"])
+    _, norm = g.finalize()
+    assert np.allclose(norm, ref["norm"], rtol=1e-6, atol=0)
+    assert g.last_launches() > 0
+
+
+@pytest.mark.parametrize("name", ["cfg2s", "cfg5s"])
+def test_grid_matches_oracle_injected_bank(name, runs, torch_cuda):
+    """Isolates the gridder: both sides use the oracle's bank (rounded to complex64 for the GPU)."""
+    wl, ref = runs(name)
+    g = make_gridder(wl)
+    g.debug_set_wkernels(wl["w_max"], ref["bank"].astype(np.complex64))
+    uvw, bl, vis, wt = to_dev(torch_cuda, wl)
+    g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+    check_grid(g.grid_complex(), ref["grid"])
+
+
+def test_row_order_and_additivity(runs, torch_cuda):
+    """Rows in random order, fed as two calls: same grid (ingest orders them; ig_grid adds)."""
+    wl, ref = runs("cfg2s")
+    rng = np.random.default_rng(5)
+    perm = rng.permutation(wl["uvw_m"].shape[0])
+    half = perm.size // 2 + 7
+    g = make_gridder(wl)
+    g.build_wkernels(wl["w_max"])
+    for part in (perm[:half], perm[half:]):
+        sub = dict(wl, uvw_m=np.ascontiguousarray(wl["uvw_m"][part]), baseline=np.ascontiguousarray(wl["baseline"][part]),
+                   vis=np.ascontiguousarray(wl["vis"][part]), weights=np.ascontiguousarray(wl["weights"][part]))
+        uvw, bl, vis, wt = to_dev(torch_cuda, sub)
+        g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+    check_grid(g.grid_complex(), ref["grid"])
+    assert g.stats() == tuple(int(x) for x in ref["stats"])
+
+
+def test_dropped_records_and_zero_weights(orc, torch_cuda):
+    """Footprints that leave the grid are dropped whole (:1278); all-zero weights drop the record (:1315)."""
+    cfg = small(synth.CONFIGS[1], n_station=8, n_time=70, n_chan=4, n_wplanes=6)
+    wl = synth.make_workload(cfg)
+    wl["cell_rad"] *= 1.8                       # shrink the uv cell: the outer tracks fall off the grid
+    wl["du"] = 1.0 / (cfg.grid_n * wl["cell_rad"])
+    wl["weights"][::3] = 0.0
+    wl["weights"][1::5, :, 1] = 0.0
+    ref = oracle_run(orc, wl)
+    assert ref["stats"][1] > 0 and ref["stats"][0] > 0
+    assert (ref["idx"]["flags"] & 2).min() == 0
+    g = make_gridder(wl)
+    g.debug_set_wkernels(wl["w_max"], ref["bank"].astype(np.complex64))
+    uvw, bl, vis, wt = to_dev(torch_cuda, wl)
+    g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+    check_grid(g.grid_complex(), ref["grid"])
+    assert g.stats() == tuple(int(x) for x in ref["stats"])
+
+
+def test_host_entry_point_and_empty_input(runs, torch_cuda):
+    wl, ref = runs("cfg1")
+    g = make_gridder(wl)
+    g.build_wkernels(wl["w_max"])
+    uvw, bl, vis, wt = to_dev(torch_cuda, wl)
+    g.grid_visibilities(uvw[:0], bl[:0], wl["freqs_hz"], vis[:0], wt[:0])     # empty batch: no work, no error
+    assert g.stats() == (0, 0, 0)
+    g.grid_visibilities_host(wl["uvw_m"], wl["baseline"], wl["freqs_hz"], np.ascontiguousarray(wl["vis"]), wl["weights"])
+    check_grid(g.grid_complex(), ref["grid"])
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2s"])
+def test_finalize_matches_oracle(name, runs, orc, torch_cuda):
+    wl, ref = runs(name)
+    cfg = wl["cfg"]
+    g = make_gridder(wl)
+    g.debug_set_wkernels(wl["w_max"], ref["bank"].astype(np.complex64))
+    uvw, bl, vis, wt = to_dev(torch_cuda, wl)
+    g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+    img, norm = g.finalize()
+    want = orc.finalize(ref["grid"], ref["norm"], cfg.oversampling)
+    got = img.cpu().numpy().astype(np.float64)
+    n = cfg.grid_n
+    inner = slice(n // 8, n - n // 8)          # the taper correction blows rounding up towards the edge
+    scale = np.abs(want[:, inner, inner]).max()
+    assert np.abs(got[:, inner, inner] - want[:, inner, inner]).max() <= 2e-4 * scale
+
+
+def test_errors_are_statuses(torch_cuda):
+    from paper_1403_4209_b200.binding import Gridder, IgError
+    with pytest.raises(IgError):
+        Gridder(255, 1e-4, 1, 8, 7, 1)          # odd grid
+    with pytest.raises(IgError):
+        Gridder(256, 1e-4, 1, 8, 8, 1)          # even support
+    g = Gridder(256, 1e-4, 1, 8, 7, 1)
+    with pytest.raises(IgError):
+        g.stats()                               # not bound yet
