@@ -127,9 +127,16 @@ ig_status ig_finalize(ig_ctx* ctx, float* image_dev, double* normaliser_host);
 /* eq 4.17: records gridded, records dropped, grid-point updates = sum S^2 * n_pol.
  * Cumulative over ig_grid calls. Synchronises. Any pointer may be NULL. */
 ig_status ig_get_stats(ig_ctx* ctx, long long* n_gridded, long long* n_dropped, long long* n_updates);
-/* Device time split of the LAST ig_grid call in milliseconds (CUDA events recorded on the
- * bound stream): ingest (A1-A3) and gridder (C). Synchronises. */
-ig_status ig_get_timing(ig_ctx* ctx, float* ingest_ms, float* gridder_ms);
+/* Pixel commits so far: atomic reductions of one multi-polarised pixel into the grid (the
+ * gridder's red.global.add traffic, for the roofline's byte count). Synchronises. */
+ig_status ig_get_commits(ig_ctx* ctx, long long* n_commits);
+/* Measured FP32 FMA peak of the device in TFLOP/s (register-only FFMA loop on every SM, timed
+ * with CUDA events on `cuda_stream`): the ALU denominator of the gridding roofline. */
+ig_status ig_measure_fp32_peak(void* cuda_stream, double* tflops);
+/* Device time split of an ig_grid call in milliseconds (CUDA events recorded on the bound
+ * stream): ingest (A1-A3) and gridder (C). calls_back = 0 is the last non-empty call, 1 the one
+ * before, ... up to 63. Waits for that call to finish. */
+ig_status ig_get_timing(ig_ctx* ctx, int calls_back, float* ingest_ms, float* gridder_ms);
 /* Zero the normaliser and the statistics (for a caller that zeroes the grid to start a new
  * image with the same bank). Asynchronous. */
 ig_status ig_reset_accumulators(ig_ctx* ctx);

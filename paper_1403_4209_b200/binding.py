@@ -35,7 +35,9 @@ SIGNATURES = {
     "ig_grid_host": (_i, [_vp, _vp, _vp, _ll, _vp, _i, _vp, _vp]),
     "ig_finalize": (_i, [_vp, _vp, _vp]),
     "ig_get_stats": (_i, [_vp, C.POINTER(_ll), C.POINTER(_ll), C.POINTER(_ll)]),
-    "ig_get_timing": (_i, [_vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]),
+    "ig_get_commits": (_i, [_vp, C.POINTER(_ll)]),
+    "ig_measure_fp32_peak": (_i, [_vp, C.POINTER(_d)]),
+    "ig_get_timing": (_i, [_vp, _i, C.POINTER(C.c_float), C.POINTER(C.c_float)]),
     "ig_reset_accumulators": (_i, [_vp]),
     "ig_last_launches": (_i, [_vp]),
     "ig_debug_indices": (_i, [_vp, _vp, _ll, _vp, _i, _vp, _vp, _vp, _vp, _vp, _vp]),
@@ -189,9 +191,20 @@ class Gridder:
         self._check(self.lib.ig_get_stats(self.ctx, C.byref(g), C.byref(d), C.byref(u)), "ig_get_stats")
         return g.value, d.value, u.value
 
-    def timing(self):
+    def commits(self) -> int:
+        n = _ll()
+        self._check(self.lib.ig_get_commits(self.ctx, C.byref(n)), "ig_get_commits")
+        return n.value
+
+    def measure_fp32_peak(self) -> float:
+        v = _d()
+        self._check(self.lib.ig_measure_fp32_peak(self._stream_ptr(), C.byref(v)), "ig_measure_fp32_peak")
+        return v.value
+
+    def timing(self, calls_back=0):
+        """(ingest_ms, gridder_ms) of the ig_grid call `calls_back` calls ago."""
         a, b = C.c_float(), C.c_float()
-        self._check(self.lib.ig_get_timing(self.ctx, C.byref(a), C.byref(b)), "ig_get_timing")
+        self._check(self.lib.ig_get_timing(self.ctx, calls_back, C.byref(a), C.byref(b)), "ig_get_timing")
         return a.value, b.value
 
     def reset(self):

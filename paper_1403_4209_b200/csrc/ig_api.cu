@@ -87,7 +87,7 @@ ig_status ig_create(ig_ctx** out, int grid_n, double cell_rad, int n_wplanes, in
 
 void ig_destroy(ig_ctx* c) {
     if (!c) return;
-    for (auto& e : c->ev) if (e) cudaEventDestroy(e);
+    for (auto& t : c->ev) for (auto& e : t) if (e) cudaEventDestroy(e);
     delete c;
 }
 
@@ -132,8 +132,9 @@ ig_status ig_bind(ig_ctx* c, void* grid_dev, size_t grid_bytes, void* work_dev, 
         cudaError_t e = cudaMemsetAsync(c->d_acc, 0, sizeof(IgAccum), c->stream);
         if (e != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_bind: ") + cudaGetErrorString(e));
     }
-    for (auto& ev : c->ev)
-        if (!ev && cudaEventCreate(&ev) != cudaSuccess) return fail(c, IG_ECUDA, "cudaEventCreate failed");
+    for (auto& t : c->ev)
+        for (auto& ev : t)
+            if (!ev && cudaEventCreate(&ev) != cudaSuccess) return fail(c, IG_ECUDA, "cudaEventCreate failed");
     c->bound = true;
     return IG_OK;
 }
@@ -193,7 +194,6 @@ ig_status ig_grid(ig_ctx* c, const double* uvw, const int* baseline_id, long lon
     if (!c->bound || !c->have_bank) return fail(c, IG_ESTATE, "ig_bind and ig_build_wkernels first");
     if (nrow < 0 || nchan < 1 || !freqs) return fail(c, IG_EINVAL, "bad nrow/nchan/freqs");
     c->launches = 0;
-    c->timed = false;
     if (nrow == 0) return IG_OK;
     if (!uvw || !baseline_id || !vis || !wt) return fail(c, IG_EINVAL, "null input");
     GridLayout L = grid_layout(c, nrow, nchan);
@@ -202,7 +202,8 @@ ig_status ig_grid(ig_ctx* c, const double* uvw, const int* baseline_id, long lon
     uint32_t* perm = (uint32_t*)(c->work + L.perm);
     uint32_t* smax = (uint32_t*)(c->work + L.smax);
     char* records = c->work + L.records;
-    cudaError_t e = cudaEventRecord(c->ev[0], c->stream);
+    cudaEvent_t* ev = c->ev[c->n_timed % IG_TIMING_RING];
+    cudaError_t e = cudaEventRecord(ev[0], c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_freqs, freqs, (size_t)nchan * 8, cudaMemcpyHostToDevice, c->stream);
     if (e != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_grid: ") + cudaGetErrorString(e));
     int n = ig_launch_sort_rows(c, baseline_id, nrow, perm, c->work + L.sort, ig_sort_scratch_bytes(nrow));
@@ -211,12 +212,12 @@ ig_status ig_grid(ig_ctx* c, const double* uvw, const int* baseline_id, long lon
     n = ig_launch_index(c, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, smax);
     if (n < 0) return IG_ECUDA;
     c->launches += n;
-    cudaEventRecord(c->ev[1], c->stream);
+    cudaEventRecord(ev[1], c->stream);
     n = ig_launch_gridder(c, records, smax, L.n_chunks);
     if (n < 0) return IG_ECUDA;
     c->launches += n;
-    cudaEventRecord(c->ev[2], c->stream);
-    c->timed = true;
+    cudaEventRecord(ev[2], c->stream);
+    c->n_timed += 1;
     return IG_OK;
 }
 
@@ -264,13 +265,25 @@ ig_status ig_get_stats(ig_ctx* c, long long* g, long long* d, long long* u) {
     return IG_OK;
 }
 
-ig_status ig_get_timing(ig_ctx* c, float* ingest_ms, float* gridder_ms) {
-    if (!c) return IG_EINVAL;
-    if (!c->timed) return fail(c, IG_ESTATE, "no timed ig_grid call");
-    if (cudaEventSynchronize(c->ev[2]) != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_get_timing: ") + cudaGetErrorString(cudaGetLastError()));
+ig_status ig_get_commits(ig_ctx* c, long long* n) {
+    if (!c || !n) return IG_EINVAL;
+    if (!c->bound) return fail(c, IG_ESTATE, "ig_bind first");
+    IgAccum a;
+    if (cudaMemcpyAsync(&a, c->d_acc, sizeof(a), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess)
+        return fail(c, IG_ECUDA, std::string("ig_get_commits: ") + cudaGetErrorString(cudaGetLastError()));
+    *n = (long long)a.commits;
+    return IG_OK;
+}
+
+ig_status ig_get_timing(ig_ctx* c, int calls_back, float* ingest_ms, float* gridder_ms) {
+    if (!c || calls_back < 0 || calls_back >= IG_TIMING_RING) return IG_EINVAL;
+    if (c->n_timed <= calls_back) return fail(c, IG_ESTATE, "no such timed ig_grid call");
+    cudaEvent_t* ev = c->ev[(c->n_timed - 1 - calls_back) % IG_TIMING_RING];
+    if (cudaEventSynchronize(ev[2]) != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_get_timing: ") + cudaGetErrorString(cudaGetLastError()));
     float a = 0, b = 0;
-    cudaEventElapsedTime(&a, c->ev[0], c->ev[1]);
-    cudaEventElapsedTime(&b, c->ev[1], c->ev[2]);
+    cudaEventElapsedTime(&a, ev[0], ev[1]);
+    cudaEventElapsedTime(&b, ev[1], ev[2]);
     if (ingest_ms) *ingest_ms = a;
     if (gridder_ms) *gridder_ms = b;
     return IG_OK;

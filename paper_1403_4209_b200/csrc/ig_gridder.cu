@@ -64,7 +64,8 @@ __device__ __forceinline__ void commit(float* __restrict__ grid, int pix, float 
 template <int NPOL>
 __global__ void __launch_bounds__(IG_GRID_WARPS * 32, 4)
 k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_smax, unsigned n_chunks,
-          float* __restrict__ grid, const float2* __restrict__ bank, int N, unsigned* __restrict__ ticket) {
+          float* __restrict__ grid, const float2* __restrict__ bank, int N, unsigned* __restrict__ ticket,
+          unsigned long long* __restrict__ commits) {
     constexpr int STRIDE = NPOL == 4 ? 48 : 32;
     constexpr int STAGE_BYTES = IG_STAGE * STRIDE;
     __shared__ __align__(128) char sm_rec[IG_GRID_WARPS][IG_CH * STRIDE];
@@ -80,6 +81,7 @@ k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_s
     }
     __syncwarp();
     uint32_t phase = 0;
+    unsigned n_commit = 0;
 
     for (;;) {
         unsigned chunk = 0;
@@ -158,7 +160,7 @@ k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_s
                     for (int k = 0; k < IG_RMAX; ++k) {
                         if (k < R && ij[k] != 0xffffffffu) {
                             if (pix[k] != prev[k]) {
-                                if (prev[k] >= 0) commit<NPOL>(grid, prev[k], acc[k]);
+                                if (prev[k] >= 0) { commit<NPOL>(grid, prev[k], acc[k]); ++n_commit; }
 #pragma unroll
                                 for (int e = 0; e < 2 * NPOL; ++e) acc[k][e] = 0.f;
                                 prev[k] = pix[k];
@@ -176,10 +178,12 @@ k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_s
             }
 #pragma unroll
             for (int k = 0; k < IG_RMAX; ++k)
-                if (k < R && prev[k] >= 0) commit<NPOL>(grid, prev[k], acc[k]);
+                if (k < R && prev[k] >= 0) { commit<NPOL>(grid, prev[k], acc[k]); ++n_commit; }
         }
         phase ^= 1u;
     }
+    n_commit = __reduce_add_sync(0xffffffffu, n_commit);
+    if (lane == 0 && n_commit) atomicAdd(commits, (unsigned long long)n_commit);
 }
 
 int ig_launch_gridder(ig_ctx* c, const char* records, const uint32_t* chunk_smax, long long n_chunks) {
@@ -194,9 +198,9 @@ int ig_launch_gridder(ig_ctx* c, const char* records, const uint32_t* chunk_smax
     unsigned ctas = (unsigned)(want < (long long)sms * per_sm ? want : (long long)sms * per_sm);
     dim3 g(ctas), b(IG_GRID_WARPS * 32);
     switch (c->prm.npol) {
-        case 1: k_gridder<1><<<g, b, 0, c->stream>>>(records, chunk_smax, (unsigned)n_chunks, c->grid, c->d_bank, c->prm.N, &c->d_acc->ticket); break;
-        case 2: k_gridder<2><<<g, b, 0, c->stream>>>(records, chunk_smax, (unsigned)n_chunks, c->grid, c->d_bank, c->prm.N, &c->d_acc->ticket); break;
-        default: k_gridder<4><<<g, b, 0, c->stream>>>(records, chunk_smax, (unsigned)n_chunks, c->grid, c->d_bank, c->prm.N, &c->d_acc->ticket); break;
+        case 1: k_gridder<1><<<g, b, 0, c->stream>>>(records, chunk_smax, (unsigned)n_chunks, c->grid, c->d_bank, c->prm.N, &c->d_acc->ticket, &c->d_acc->commits); break;
+        case 2: k_gridder<2><<<g, b, 0, c->stream>>>(records, chunk_smax, (unsigned)n_chunks, c->grid, c->d_bank, c->prm.N, &c->d_acc->ticket, &c->d_acc->commits); break;
+        default: k_gridder<4><<<g, b, 0, c->stream>>>(records, chunk_smax, (unsigned)n_chunks, c->grid, c->d_bank, c->prm.N, &c->d_acc->ticket, &c->d_acc->commits); break;
     }
     IG_CUDA_OK(c, cudaGetLastError());
     return 1;

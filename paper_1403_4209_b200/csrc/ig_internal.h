@@ -10,6 +10,7 @@
 #define IG_STAGE 32          // records per TMA stage
 #define IG_NSTAGE (IG_CH / IG_STAGE)
 #define IG_RMAX 8            // grid points per lane, at most
+#define IG_TIMING_RING 64    // ig_grid calls whose event triples are kept
 #define IG_GRID_WARPS 4      // warps per gridder CTA
 
 // Device-side tail of the bank buffer: small tables and accumulators.
@@ -17,6 +18,7 @@ struct IgPlaneEntry { int support; uint32_t koff; };   // koff in complex elemen
 struct IgAccum {
     double norm[4];                     // eq 4.5 normaliser per polarisation
     unsigned long long gridded, dropped, updates;   // eq 4.17
+    unsigned long long commits;         // pixel commits (atomic reductions of one multi-pol pixel) by the gridder
     unsigned int ticket;                // work queue of the gridder
     unsigned int max_key;               // largest baseline id of the current call
 };
@@ -45,8 +47,8 @@ struct ig_ctx {
     float2* d_bank = nullptr; double* d_zeta = nullptr; IgPlaneEntry* d_planes = nullptr;
     IgAccum* d_acc = nullptr;
     // timing of the last ig_grid
-    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
-    bool timed = false;
+    cudaEvent_t ev[IG_TIMING_RING][3] = {};   // ring over the last ig_grid calls
+    long long n_timed = 0;                    // ig_grid calls timed so far
     int launches = 0;
     std::string err;
 };

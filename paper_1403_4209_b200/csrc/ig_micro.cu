@@ -1,0 +1,51 @@
+// ig_micro.cu - FP32 FMA peak microbenchmark (the ALU denominator of the gridding roofline,
+// "8 FP32 flops per complex update at FP32 peak").
+// Register-only dependent-chain FFMAs, 8 independent chains per thread, enough warps per SM to
+// cover the 4-cycle FMA latency; nothing touches memory inside the loop.
+#include "ig_internal.h"
+
+__global__ void __launch_bounds__(256) k_ffma_peak(float* out, int iters, float a, float b) {
+    float x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = (float)(threadIdx.x + i);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) x[i] = fmaf(x[i], a, b);
+        }
+    }
+    float s = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += x[i];
+    if (s == 123.456f) out[0] = s;   // never true; keeps the chains alive
+}
+
+extern "C" ig_status ig_measure_fp32_peak(void* cuda_stream, double* tflops) {
+    if (!tflops) return IG_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return IG_ECUDA;
+    float* d = nullptr;   // 4-byte sink, only ever written if the impossible branch is taken
+    if (cudaMalloc(&d, 4) != cudaSuccess) return IG_ECUDA;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int iters = 20000, ctas = sms * 8, thr = 256;
+    double best = 0;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0, st);
+        k_ffma_peak<<<ctas, thr, 0, st>>>(d, iters, 1.0000001f, 1e-9f);
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d); return IG_ECUDA; }
+        float ms = 0;
+        cudaEventElapsedTime(&ms, e0, e1);
+        double fl = 2.0 * 64.0 * iters * (double)ctas * thr;
+        double t = fl / (ms * 1e-3) / 1e12;
+        if (rep > 0 && t > best) best = t;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(d);
+    *tflops = best;
+    return IG_OK;
+}
