@@ -167,35 +167,26 @@ def run_reference(args):
 
 def run_ours(args):
     import torch
-    import torch.distributed as dist
     from paper_1403_4209_b200 import build as igbuild
     from paper_1403_4209_b200.binding import Gridder
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_1403_4209_b200.dist import Ranks
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+    ranks = Ranks(backend="nccl", device=dev)
+    world, rank = ranks.world, ranks.rank
     if rank == 0:
         igbuild.build()
-    if world > 1:
-        dist.barrier()
+    ranks.barrier()
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        ranks.barrier()
         torch.cuda.synchronize(dev)
 
-    def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    max_over_ranks = ranks.max_over_ranks
 
     cfg = synth.CONFIGS[args.config - 1]
     t_gen = time.perf_counter()
@@ -273,8 +264,7 @@ def run_ours(args):
                "ms_per_step": dt * 1e3, "steps": n_e2e}
 
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
+        ranks.close()
         return
 
     # ---- roofline of the dominant kernel (k_gridder), DESIGN.md "Roofline" -------------------------
@@ -319,8 +309,7 @@ def run_ours(args):
         "context": "thesis GTX 680: ~50 G updates/s real rate, Romein 93 G (PAPER.md:742,:1986) - other hardware, not a target",
     }
     print(json.dumps(out))
-    if world > 1:
-        dist.destroy_process_group()
+    ranks.close()
 
 
 if __name__ == "__main__":

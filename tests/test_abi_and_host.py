@@ -1,0 +1,101 @@
+"""CPU-side checks of the CUDA path's host logic: the C-ABI library loads without a GPU and exports every
+symbol include/ig.h declares; argument validation; size queries; the library's taper (host code) against the
+oracle's; the replica plumbing of bench.py under gloo with world size 2."""
+import ctypes
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1403_4209_b200 import build, binding
+    build.build()
+    return binding.load()
+
+
+def test_every_declared_symbol_is_exported(lib):
+    from paper_1403_4209_b200 import binding
+    hdr = open(os.path.join(ROOT, "include", "ig.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(ig_[a-z0-9_]+)\s*\(", hdr))
+    assert len(declared) >= 20
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert declared == set(binding.SIGNATURES), declared ^ set(binding.SIGNATURES)
+
+
+def test_create_validates_arguments(lib):
+    ctx = ctypes.c_void_p()
+    ok = (256, 1e-4, 4, 8, 7, 4)
+    bad = [(255, 1e-4, 4, 8, 7, 4), (256, 0.0, 4, 8, 7, 4), (256, 1e-4, 0, 8, 7, 4), (256, 1e-4, 4, 0, 7, 4),
+           (256, 1e-4, 4, 8, 8, 4), (256, 1e-4, 4, 8, 257, 4), (256, 1e-4, 4, 8, 7, 3), (8, 1e-4, 1, 8, 7, 1)]
+    for a in bad:
+        assert lib.ig_create(ctypes.byref(ctx), *a) == 1, a
+        assert not ctx.value
+    assert lib.ig_create(ctypes.byref(ctx), *ok) == 0
+    assert lib.ig_grid_bytes(ctx) == 256 * 256 * 4 * 8
+    sup = np.array([7, 7, 5, 3], dtype=np.int32)
+    head = lib.ig_bank_bytes(ctx, sup.ctypes.data_as(ctypes.c_void_p)) - (49 + 49 + 25 + 9) * 64 * 8
+    assert 0 < head < 8192
+    assert lib.ig_bank_bytes(ctx, None) >= lib.ig_bank_bytes(ctx, sup.ctypes.data_as(ctypes.c_void_p))
+    w1, w2 = lib.ig_workspace_bytes(ctx, 1000, 4), lib.ig_workspace_bytes(ctx, 100000, 4)
+    assert w2 > w1 > 0
+    # 100000 rows -> 782 row blocks x 4 channels x 128 records x 48 B
+    assert w2 >= 782 * 4 * 128 * 48
+    # calls out of order are statuses, not crashes
+    assert lib.ig_get_stats(ctx, None, None, None) == 2
+    assert lib.ig_build_wkernels(ctx, 10.0, sup.ctypes.data_as(ctypes.c_void_p)) == 2
+    assert lib.ig_grid(ctx, None, None, 0, None, 1, None, None) == 2
+    assert b"ig_bind" in lib.ig_last_error(ctx)
+    lib.ig_destroy(ctx)
+
+
+def test_library_taper_matches_oracle(lib, orc):
+    from paper_1403_4209_b200 import binding
+    eta = np.linspace(-1.3, 1.3, 777)
+    got, want = binding.taper(eta), orc.taper(eta)
+    assert np.abs(got - want).max() < 1e-12
+    assert got[np.abs(eta) >= 1].max() == 0.0
+
+
+def test_missing_library_fails_loudly(monkeypatch, tmp_path):
+    from paper_1403_4209_b200 import binding
+    monkeypatch.setattr(binding, "_LIB", None)
+    monkeypatch.setattr(binding, "lib_path", lambda: str(tmp_path / "nope.so"))
+    with pytest.raises(binding.IgError):
+        binding.load()
+
+
+_WORKER = r"""
+import os, sys
+sys.path.insert(0, sys.argv[1])
+from paper_1403_4209_b200.dist import Ranks
+r = Ranks(backend="gloo")
+assert r.world == 2
+r.barrier()
+t = 1.0 + r.rank            # rank 1 is the slow one
+m = r.max_over_ranks(t)
+rate = r.aggregate_rate(100.0, t)
+assert m == 2.0, m
+assert rate == 2 * 100.0 / 2.0, rate
+r.close()
+print("ok", r.rank)
+"""
+
+
+def test_replica_plumbing_gloo_world2(tmp_path):
+    script = tmp_path / "w.py"
+    script.write_text(_WORKER)
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29731")
+    out = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                          "--master-addr", "127.0.0.1", "--master-port", "29731", str(script), ROOT],
+                         capture_output=True, text=True, env=env, timeout=300)
+    assert out.returncode == 0, out.stderr[-2000:]
+    assert out.stdout.count("ok") == 2
