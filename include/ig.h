@@ -133,6 +133,12 @@ ig_status ig_get_commits(ig_ctx* ctx, long long* n_commits);
 /* Measured FP32 FMA peak of the device in TFLOP/s (register-only FFMA loop on every SM, timed
  * with CUDA events on `cuda_stream`): the ALU denominator of the gridding roofline. */
 ig_status ig_measure_fp32_peak(void* cuda_stream, double* tflops);
+/* Measured rate of the gridder's commit (one 32-byte 4-pol pixel = 2 x red.global.add.v4.f32) at
+ * pseudo-random places of buf_dev (dev, `bytes` long, contents are added to), in 1e9 pixel commits/s.
+ * run_len = consecutive pixels committed by neighbouring lanes (1..32). The atomic ceiling of the
+ * roofline: L2-resident when bytes << 126 MB, HBM-backed when bytes >> 126 MB. */
+ig_status ig_measure_commit_rate(void* cuda_stream, void* buf_dev, size_t bytes, int run_len,
+                                 double* gcommits_per_s);
 /* Device time split of an ig_grid call in milliseconds (CUDA events recorded on the bound
  * stream): ingest (A1-A3) and gridder (C). calls_back = 0 is the last non-empty call, 1 the one
  * before, ... up to 63. Waits for that call to finish. */

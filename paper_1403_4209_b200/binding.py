@@ -37,6 +37,7 @@ SIGNATURES = {
     "ig_get_stats": (_i, [_vp, C.POINTER(_ll), C.POINTER(_ll), C.POINTER(_ll)]),
     "ig_get_commits": (_i, [_vp, C.POINTER(_ll)]),
     "ig_measure_fp32_peak": (_i, [_vp, C.POINTER(_d)]),
+    "ig_measure_commit_rate": (_i, [_vp, _vp, _sz, _i, C.POINTER(_d)]),
     "ig_get_timing": (_i, [_vp, _i, C.POINTER(C.c_float), C.POINTER(C.c_float)]),
     "ig_reset_accumulators": (_i, [_vp]),
     "ig_last_launches": (_i, [_vp]),
@@ -199,6 +200,14 @@ class Gridder:
     def measure_fp32_peak(self) -> float:
         v = _d()
         self._check(self.lib.ig_measure_fp32_peak(self._stream_ptr(), C.byref(v)), "ig_measure_fp32_peak")
+        return v.value
+
+    def measure_commit_rate(self, nbytes, run_len=8) -> float:
+        """1e9 pixel commits/s into a scratch buffer of nbytes (see include/ig.h)."""
+        buf = self.torch.zeros(int(nbytes) // 4, dtype=self.torch.float32, device=self.device)
+        v = _d()
+        self._check(self.lib.ig_measure_commit_rate(self._stream_ptr(), _vp(buf.data_ptr()), buf.numel() * 4, run_len,
+                                                    C.byref(v)), "ig_measure_commit_rate")
         return v.value
 
     def timing(self, calls_back=0):

@@ -49,3 +49,48 @@ extern "C" ig_status ig_measure_fp32_peak(void* cuda_stream, double* tflops) {
     *tflops = best;
     return IG_OK;
 }
+
+// ---------------------------------------------------------------------------------------------
+// Pixel-commit microbenchmark: the gridder's commit (2 x red.global.add.v4.f32 = one 32-byte 4-pol
+// pixel) issued at pseudo-random pixels of a caller-provided buffer, nothing else in the loop. Gives the
+// L2 atomic ceiling (buffer resident in L2) and the HBM-backed ceiling (buffer far larger than L2) that
+// the byte side of the gridding roofline is compared with.
+__global__ void __launch_bounds__(256) k_red_rate(float* buf, unsigned long long n_pix, int iters, unsigned run_len) {
+    unsigned long long x = 0x9E3779B97F4A7C15ull * (blockIdx.x * 256ull + threadIdx.x + 1);
+    for (int it = 0; it < iters; ++it) {
+        x ^= x << 13; x ^= x >> 7; x ^= x << 17;
+        // run_len consecutive pixels per random start, lanes of a warp on consecutive pixels: the
+        // gridder's pattern (a warp commits a run of neighbouring pixels of one footprint row)
+        unsigned long long start = __shfl_sync(0xffffffffu, x, 0) % n_pix;
+        unsigned long long pix = (start + (threadIdx.x & 31) % run_len + ((threadIdx.x & 31) / run_len) * 4099ull) % n_pix;
+        float* g = buf + pix * 8;
+        asm volatile("red.global.add.v4.f32 [%0], {%1,%1,%1,%1};" ::"l"(g), "f"(1.0f) : "memory");
+        asm volatile("red.global.add.v4.f32 [%0], {%1,%1,%1,%1};" ::"l"(g + 4), "f"(1.0f) : "memory");
+    }
+}
+
+extern "C" ig_status ig_measure_commit_rate(void* cuda_stream, void* buf_dev, size_t bytes, int run_len,
+                                            double* gcommits_per_s) {
+    if (!buf_dev || bytes < 4096 || !gcommits_per_s || run_len < 1 || run_len > 32) return IG_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return IG_ECUDA;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int iters = 2000, ctas = sms * 8;
+    double best = 0;
+    for (int rep = 0; rep < 3; ++rep) {
+        cudaEventRecord(e0, st);
+        k_red_rate<<<ctas, 256, 0, st>>>((float*)buf_dev, bytes / 32, iters, (unsigned)run_len);
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess) return IG_ECUDA;
+        float ms = 0;
+        cudaEventElapsedTime(&ms, e0, e1);
+        double r = (double)iters * ctas * 256 / (ms * 1e-3) / 1e9;
+        if (rep > 0 && r > best) best = r;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    *gcommits_per_s = best;
+    return IG_OK;
+}
