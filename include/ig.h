@@ -130,6 +130,9 @@ ig_status ig_get_stats(ig_ctx* ctx, long long* n_gridded, long long* n_dropped, 
 /* Pixel commits so far: atomic reductions of one multi-polarised pixel into the grid (the
  * gridder's red.global.add traffic, for the roofline's byte count). Synchronises. */
 ig_status ig_get_commits(ig_ctx* ctx, long long* n_commits);
+/* Counting costs a few instructions per grid point and record, so it is off by default: switch it on for
+ * the ig_grid calls whose commits are to be counted (bench.py's counted pass). */
+ig_status ig_set_commit_counting(ig_ctx* ctx, int on);
 /* Measured FP32 FMA peak of the device in TFLOP/s (register-only FFMA loop on every SM, timed
  * with CUDA events on `cuda_stream`): the ALU denominator of the gridding roofline. */
 ig_status ig_measure_fp32_peak(void* cuda_stream, double* tflops);

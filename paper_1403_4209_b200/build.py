@@ -32,6 +32,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
            "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES] + [
            "-L" + os.path.join(CUDA_HOME, "lib64"), "-lcufft",
            "-Xlinker", "-rpath," + os.path.join(CUDA_HOME, "lib64")]
+    cmd[1:1] = os.environ.get("IG_NVCC_EXTRA", "").split()   # tuning experiments only (-DIG_RMAX=.. etc.)
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     subprocess.check_call(cmd)

@@ -206,14 +206,16 @@ ig_status ig_grid(ig_ctx* c, const double* uvw, const int* baseline_id, long lon
     cudaError_t e = cudaEventRecord(ev[0], c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_freqs, freqs, (size_t)nchan * 8, cudaMemcpyHostToDevice, c->stream);
     if (e != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_grid: ") + cudaGetErrorString(e));
-    int n = ig_launch_sort_rows(c, baseline_id, nrow, perm, c->work + L.sort, ig_sort_scratch_bytes(nrow));
+    double fref = 0;
+    for (int k = 0; k < nchan; ++k) fref += freqs[k] / nchan;
+    int n = ig_launch_sort_rows(c, uvw, baseline_id, nrow, fref, perm, c->work + L.sort, ig_sort_scratch_bytes(nrow));
     if (n < 0) return IG_ECUDA;
     c->launches += n;
     n = ig_launch_index(c, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, smax);
     if (n < 0) return IG_ECUDA;
     c->launches += n;
     cudaEventRecord(ev[1], c->stream);
-    n = ig_launch_gridder(c, records, smax, L.n_chunks);
+    n = ig_launch_gridder(c, records, smax, L.nrb, nchan);
     if (n < 0) return IG_ECUDA;
     c->launches += n;
     cudaEventRecord(ev[2], c->stream);
@@ -262,6 +264,12 @@ ig_status ig_get_stats(ig_ctx* c, long long* g, long long* d, long long* u) {
     if (g) *g = (long long)a.gridded;
     if (d) *d = (long long)a.dropped;
     if (u) *u = (long long)a.updates;
+    return IG_OK;
+}
+
+ig_status ig_set_commit_counting(ig_ctx* c, int on) {
+    if (!c) return IG_EINVAL;
+    c->count_commits = on != 0;
     return IG_OK;
 }
 

@@ -49,6 +49,56 @@ __device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t
                  : "memory");
 }
 
+// Commit step of one owned point, branch-free: if the record's pixel differs from the one the lane
+// holds, the held sums go to the grid with vector reductions (unless the lane held nothing, prev < 0),
+// the sums restart from zero and the lane takes the new pixel. Written as predicated PTX so that the
+// sums stay in place (the compiler's own if-conversion copied all eight registers per point and record)
+// and no BSSY/BSYNC pair is issued. COUNT adds the commit counter (ig_get_commits).
+template <int NPOL, bool COUNT>
+__device__ __forceinline__ void commit_step(float (&a)[2 * NPOL], int& prev, int pix, float* __restrict__ grid,
+                                            unsigned& n_commit) {
+    if constexpr (COUNT) n_commit += (pix != prev && prev >= 0) ? 1u : 0u;
+    if constexpr (NPOL == 4) {
+        asm volatile(
+            "{\n\t.reg .pred p, q;\n\t.reg .u64 ad;\n\t"
+            "setp.ne.s32 p, %9, %8;\n\t"
+            "setp.ge.and.s32 q, %8, 0, p;\n\t"
+            "@q mad.wide.s32 ad, %8, 32, %10;\n\t"
+            "@q red.global.add.v4.f32 [ad], {%0,%1,%2,%3};\n\t"
+            "@q red.global.add.v4.f32 [ad+16], {%4,%5,%6,%7};\n\t"
+            "@p mov.f32 %0, 0f00000000;\n\t@p mov.f32 %1, 0f00000000;\n\t@p mov.f32 %2, 0f00000000;\n\t"
+            "@p mov.f32 %3, 0f00000000;\n\t@p mov.f32 %4, 0f00000000;\n\t@p mov.f32 %5, 0f00000000;\n\t"
+            "@p mov.f32 %6, 0f00000000;\n\t@p mov.f32 %7, 0f00000000;\n\t"
+            "@p mov.s32 %8, %9;\n\t}"
+            : "+f"(a[0]), "+f"(a[1]), "+f"(a[2]), "+f"(a[3]), "+f"(a[4]), "+f"(a[5]), "+f"(a[6]), "+f"(a[7]), "+r"(prev)
+            : "r"(pix), "l"(grid));
+    } else if constexpr (NPOL == 2) {
+        asm volatile(
+            "{\n\t.reg .pred p, q;\n\t.reg .u64 ad;\n\t"
+            "setp.ne.s32 p, %5, %4;\n\t"
+            "setp.ge.and.s32 q, %4, 0, p;\n\t"
+            "@q mad.wide.s32 ad, %4, 16, %6;\n\t"
+            "@q red.global.add.v4.f32 [ad], {%0,%1,%2,%3};\n\t"
+            "@p mov.f32 %0, 0f00000000;\n\t@p mov.f32 %1, 0f00000000;\n\t@p mov.f32 %2, 0f00000000;\n\t"
+            "@p mov.f32 %3, 0f00000000;\n\t"
+            "@p mov.s32 %4, %5;\n\t}"
+            : "+f"(a[0]), "+f"(a[1]), "+f"(a[2]), "+f"(a[3]), "+r"(prev)
+            : "r"(pix), "l"(grid));
+    } else {
+        asm volatile(
+            "{\n\t.reg .pred p, q;\n\t.reg .u64 ad;\n\t"
+            "setp.ne.s32 p, %3, %2;\n\t"
+            "setp.ge.and.s32 q, %2, 0, p;\n\t"
+            "@q mad.wide.s32 ad, %2, 8, %4;\n\t"
+            "@q red.global.add.v2.f32 [ad], {%0,%1};\n\t"
+            "@p mov.f32 %0, 0f00000000;\n\t@p mov.f32 %1, 0f00000000;\n\t"
+            "@p mov.s32 %2, %3;\n\t}"
+            : "+f"(a[0]), "+f"(a[1]), "+r"(prev)
+            : "r"(pix), "l"(grid));
+    }
+}
+
+// final flush of one point
 template <int NPOL>
 __device__ __forceinline__ void commit(float* __restrict__ grid, int pix, float (&a)[2 * NPOL]) {
     float* g = grid + (size_t)pix * (2 * NPOL);
@@ -61,9 +111,75 @@ __device__ __forceinline__ void commit(float* __restrict__ grid, int pix, float 
     }
 }
 
-template <int NPOL>
-__global__ void __launch_bounds__(IG_GRID_WARPS * 32, 4)
-k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_smax, unsigned n_chunks,
+// One pass of one warp over a RUN of records of equal support S (contiguous in the staged item):
+// the lane owns the R points q = q0 + 32k of the S x S footprint. Control flow is warp-uniform.
+// Lanes whose q lies outside the footprint run the same instructions on tap (0,0) with the sentinel
+// pixel -1, which never commits.
+template <int NPOL, int R, bool COUNT>
+__device__ __forceinline__ unsigned grid_run(const char* __restrict__ rp, int n_rec, int S, int q0,
+                                             float* __restrict__ grid, const float2* __restrict__ bank, int N) {
+    constexpr int STRIDE = NPOL == 4 ? 48 : 32;
+    float acc[R][2 * NPOL];
+    int prev[R], ii[R], jj[R];
+    uint32_t amask = 0;
+#pragma unroll
+    for (int k = 0; k < R; ++k) {
+        const int q = q0 + k * 32;
+        const int j = q / S;
+        const bool act = q < S * S;
+        ii[k] = act ? q - j * S : 0;
+        jj[k] = act ? j : 0;
+        amask |= act ? (1u << k) : 0u;
+        prev[k] = -1;
+#pragma unroll
+        for (int e = 0; e < 2 * NPOL; ++e) acc[k][e] = 0.f;
+    }
+    unsigned n_commit = 0;
+#pragma unroll 1
+    for (int r = 0; r < n_rec; ++r, rp += STRIDE) {
+        const uint4 h = *reinterpret_cast<const uint4*>(rp);
+        const int cm = (int)(h.z & 0xffu), dm = (int)((h.z >> 8) & 0xffu);
+        float v[2 * NPOL];
+        {
+            const float4 a = *reinterpret_cast<const float4*>(rp + 16);
+            v[0] = a.x; v[1] = a.y;
+            if constexpr (NPOL >= 2) { v[2] = a.z; v[3] = a.w; }
+            if constexpr (NPOL == 4) {
+                const float4 b = *reinterpret_cast<const float4*>(rp + 32);
+                v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+            }
+        }
+        float2 kv[R];
+        int pix[R];
+#pragma unroll
+        for (int k = 0; k < R; ++k) {
+            const int tu = ii[k] + cm, tv = jj[k] + dm;
+            const int tx = (int)min((unsigned)tu, (unsigned)(tu - S));     // (i + c) mod S
+            const int ty = (int)min((unsigned)tv, (unsigned)(tv - S));
+            pix[k] = (amask & (1u << k)) ? ty * N + ((int)h.x + tx) : -1;
+            kv[k] = __ldg(bank + (uint32_t)(ty * S + (tx + (int)h.y)));   // 32-bit element index
+        }
+#pragma unroll
+        for (int k = 0; k < R; ++k) {
+            commit_step<NPOL, COUNT>(acc[k], prev[k], pix[k], grid, n_commit);
+#pragma unroll
+            for (int q = 0; q < NPOL; ++q) {
+                acc[k][2 * q] = fmaf(v[2 * q], kv[k].x, acc[k][2 * q]);
+                acc[k][2 * q] = fmaf(-v[2 * q + 1], kv[k].y, acc[k][2 * q]);
+                acc[k][2 * q + 1] = fmaf(v[2 * q], kv[k].y, acc[k][2 * q + 1]);
+                acc[k][2 * q + 1] = fmaf(v[2 * q + 1], kv[k].x, acc[k][2 * q + 1]);
+            }
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < R; ++k)
+        if (prev[k] >= 0) { commit<NPOL>(grid, prev[k], acc[k]); ++n_commit; }
+    return n_commit;
+}
+
+template <int NPOL, bool COUNT>
+__global__ void __launch_bounds__(IG_GRID_WARPS * 32, IG_GRID_CTAS_PER_SM)
+k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_smax, unsigned nrb, unsigned nchan,
           float* __restrict__ grid, const float2* __restrict__ bank, int N, unsigned* __restrict__ ticket,
           unsigned long long* __restrict__ commits) {
     constexpr int STRIDE = NPOL == 4 ? 48 : 32;
@@ -82,15 +198,18 @@ k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_s
     __syncwarp();
     uint32_t phase = 0;
     unsigned n_commit = 0;
+    const unsigned n_chunks = nrb * nchan;
 
     for (;;) {
-        unsigned chunk = 0;
-        if (lane == 0) chunk = atomicAdd(ticket, 1u);
-        chunk = __shfl_sync(0xffffffffu, chunk, 0);
-        if (chunk >= n_chunks) break;
-        const int smax = (int)chunk_smax[chunk];
-        if (smax == 0) continue;                       // every record of the item was dropped
-        __syncwarp();                                  // all lanes are done with the previous chunk
+        unsigned tk = 0;
+        if (lane == 0) tk = atomicAdd(ticket, 1u);
+        tk = __shfl_sync(0xffffffffu, tk, 0);
+        if (tk >= n_chunks) break;
+        // tickets run channel-major: neighbours in the queue are neighbouring row blocks of ONE channel
+        const unsigned ch = tk / nrb;
+        const unsigned chunk = (tk - ch * nrb) * nchan + ch;
+        if (chunk_smax[chunk] == 0) continue;          // every record of the item was dropped
+        __syncwarp();                                  // all lanes are done with the previous item
         if (lane == 0) {
             const char* src = records + (size_t)chunk * (IG_CH * STRIDE);
 #pragma unroll
@@ -99,109 +218,92 @@ k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_s
                 tma_load_1d(my_rec + s * STAGE_BYTES, src + s * STAGE_BYTES, STAGE_BYTES, &my_bar[s]);
             }
         }
-        const int s2max = smax * smax;
-        const int n_pass = (s2max + 32 * IG_RMAX - 1) / (32 * IG_RMAX);
-        const int R = (s2max + 32 * n_pass - 1) / (32 * n_pass);   // points per lane, <= IG_RMAX
-
-        for (int pass = 0; pass < n_pass; ++pass) {
-            const int q0 = pass * 32 * R + lane;
-            float acc[IG_RMAX][2 * NPOL];
-            int prev[IG_RMAX];
-            uint32_t ij[IG_RMAX];
+        // Cut the item into runs of equal support. A support change re-maps every lane's residues, so all
+        // points commit there anyway (Romein's scheme flushes on a support change too); per
+        // run the pass count and R are then the best fit for that support, not for the item's largest one.
+        uint32_t bnd[IG_NSTAGE];                       // bit r of bnd[g]: record 32g+r starts a run
+        int s_prev = -1;
 #pragma unroll
-            for (int k = 0; k < IG_RMAX; ++k) {
-                prev[k] = -1; ij[k] = 0xffffffffu;
+        for (int g = 0; g < IG_NSTAGE; ++g) {
+            mbar_wait(&my_bar[g], phase);
+            const int sv = (int)((*reinterpret_cast<const uint32_t*>(my_rec + (g * 32 + lane) * STRIDE + 8) >> 16) & 0xffu);
+            int before = __shfl_up_sync(0xffffffffu, sv, 1);
+            if (lane == 0) before = s_prev;
+            bnd[g] = __ballot_sync(0xffffffffu, sv != before);
+            s_prev = __shfl_sync(0xffffffffu, sv, 31);
+        }
+        int r0 = 0;
+        while (r0 < IG_CH) {
+            // end of the run that starts at r0: the next boundary bit after r0
+            int r1 = IG_CH;
 #pragma unroll
-                for (int e = 0; e < 2 * NPOL; ++e) acc[k][e] = 0.f;
+            for (int g = IG_NSTAGE - 1; g >= 0; --g) {
+                uint32_t m = bnd[g];
+                const int lo = r0 + 1 - g * 32;        // first bit of this word that lies after r0
+                if (lo >= 32) m = 0u;
+                else if (lo > 0) m &= 0xffffffffu << lo;
+                if (m) r1 = g * 32 + __ffs(m) - 1;     // lower words are visited last: smallest wins
             }
-            int curS = 0;
-            for (int st = 0; st < IG_NSTAGE; ++st) {
-                if (pass == 0) mbar_wait(&my_bar[st], phase);
-                const char* rp = my_rec + st * STAGE_BYTES;
-                for (int r = 0; r < IG_STAGE; ++r, rp += STRIDE) {
-                    const uint4 h = *reinterpret_cast<const uint4*>(rp);
-                    const int S = (int)((h.z >> 16) & 0xffu);
-                    if (S == 0) continue;              // dropped record (step A3)
-                    if (S != curS) {                   // new support: re-derive the owned residues
-                        curS = S;
-#pragma unroll
-                        for (int k = 0; k < IG_RMAX; ++k) {
-                            if (k < R) {
-                                const int q = q0 + k * 32;
-                                const int j = q / S;
-                                ij[k] = (q < S * S) ? (uint32_t)((q - j * S) | (j << 8)) : 0xffffffffu;
-                            }
-                        }
-                    }
-                    const int cm = (int)(h.z & 0xffu), dm = (int)((h.z >> 8) & 0xffu);
-                    float v[2 * NPOL];
-                    {
-                        const float4 a = *reinterpret_cast<const float4*>(rp + 16);
-                        v[0] = a.x; v[1] = a.y;
-                        if constexpr (NPOL >= 2) { v[2] = a.z; v[3] = a.w; }
-                        if constexpr (NPOL == 4) {
-                            const float4 b = *reinterpret_cast<const float4*>(rp + 32);
-                            v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
-                        }
-                    }
-                    const float2* kb = bank + h.y;
-                    float2 kv[IG_RMAX];
-                    int pix[IG_RMAX];
-#pragma unroll
-                    for (int k = 0; k < IG_RMAX; ++k) {
-                        if (k < R && ij[k] != 0xffffffffu) {
-                            int tx = (int)(ij[k] & 0xffu) + cm; tx = tx >= S ? tx - S : tx;
-                            int ty = (int)(ij[k] >> 8) + dm;    ty = ty >= S ? ty - S : ty;
-                            pix[k] = (int)h.x + ty * N + tx;
-                            kv[k] = __ldg(kb + ty * S + tx);
-                        }
-                    }
-#pragma unroll
-                    for (int k = 0; k < IG_RMAX; ++k) {
-                        if (k < R && ij[k] != 0xffffffffu) {
-                            if (pix[k] != prev[k]) {
-                                if (prev[k] >= 0) { commit<NPOL>(grid, prev[k], acc[k]); ++n_commit; }
-#pragma unroll
-                                for (int e = 0; e < 2 * NPOL; ++e) acc[k][e] = 0.f;
-                                prev[k] = pix[k];
-                            }
-#pragma unroll
-                            for (int q = 0; q < NPOL; ++q) {
-                                acc[k][2 * q] = fmaf(v[2 * q], kv[k].x, acc[k][2 * q]);
-                                acc[k][2 * q] = fmaf(-v[2 * q + 1], kv[k].y, acc[k][2 * q]);
-                                acc[k][2 * q + 1] = fmaf(v[2 * q], kv[k].y, acc[k][2 * q + 1]);
-                                acc[k][2 * q + 1] = fmaf(v[2 * q + 1], kv[k].x, acc[k][2 * q + 1]);
-                            }
-                        }
+            const char* rp = my_rec + r0 * STRIDE;
+            const int S = (int)((*reinterpret_cast<const uint32_t*>(rp + 8) >> 16) & 0xffu);
+            if (S != 0) {
+                const int s2 = S * S;
+                const int n_pass = (s2 + 32 * IG_RMAX - 1) / (32 * IG_RMAX);
+                const int R = (s2 + 32 * n_pass - 1) / (32 * n_pass);   // points per lane, <= IG_RMAX
+                for (int pass = 0; pass < n_pass; ++pass) {
+                    const int q0 = pass * 32 * R + lane;
+                    switch (R) {
+#define IG_CASE(r) case r: n_commit += grid_run<NPOL, r, COUNT>(rp, r1 - r0, S, q0, grid, bank, N); break;
+                        IG_CASE(1) IG_CASE(2)
+#if IG_RMAX >= 3
+                        IG_CASE(3)
+#endif
+#if IG_RMAX >= 4
+                        IG_CASE(4)
+#endif
+#if IG_RMAX >= 5
+                        IG_CASE(5)
+#endif
+#if IG_RMAX >= 6
+                        IG_CASE(6)
+#endif
+#if IG_RMAX >= 8
+                        IG_CASE(7) IG_CASE(8)
+#endif
+#undef IG_CASE
+                        default: break;
                     }
                 }
             }
-#pragma unroll
-            for (int k = 0; k < IG_RMAX; ++k)
-                if (k < R && prev[k] >= 0) { commit<NPOL>(grid, prev[k], acc[k]); ++n_commit; }
+            r0 = r1;
         }
         phase ^= 1u;
     }
-    n_commit = __reduce_add_sync(0xffffffffu, n_commit);
-    if (lane == 0 && n_commit) atomicAdd(commits, (unsigned long long)n_commit);
+    if constexpr (COUNT) {
+        n_commit = __reduce_add_sync(0xffffffffu, n_commit);
+        if (lane == 0 && n_commit) atomicAdd(commits, (unsigned long long)n_commit);
+    }
 }
 
-int ig_launch_gridder(ig_ctx* c, const char* records, const uint32_t* chunk_smax, long long n_chunks) {
+int ig_launch_gridder(ig_ctx* c, const char* records, const uint32_t* chunk_smax, long long nrb, int nchan) {
+    const long long n_chunks = nrb * nchan;
     if (n_chunks == 0) return 0;
     if (n_chunks >= (1ll << 32) - 65536) { c->err = "too many work items"; return -1; }
     IG_CUDA_OK(c, cudaMemsetAsync(&c->d_acc->ticket, 0, sizeof(unsigned), c->stream));
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    int per_sm = 4;
+    int per_sm = IG_GRID_CTAS_PER_SM;
     long long want = (n_chunks + IG_GRID_WARPS - 1) / IG_GRID_WARPS;
     unsigned ctas = (unsigned)(want < (long long)sms * per_sm ? want : (long long)sms * per_sm);
     dim3 g(ctas), b(IG_GRID_WARPS * 32);
-    switch (c->prm.npol) {
-        case 1: k_gridder<1><<<g, b, 0, c->stream>>>(records, chunk_smax, (unsigned)n_chunks, c->grid, c->d_bank, c->prm.N, &c->d_acc->ticket, &c->d_acc->commits); break;
-        case 2: k_gridder<2><<<g, b, 0, c->stream>>>(records, chunk_smax, (unsigned)n_chunks, c->grid, c->d_bank, c->prm.N, &c->d_acc->ticket, &c->d_acc->commits); break;
-        default: k_gridder<4><<<g, b, 0, c->stream>>>(records, chunk_smax, (unsigned)n_chunks, c->grid, c->d_bank, c->prm.N, &c->d_acc->ticket, &c->d_acc->commits); break;
+#define IG_LAUNCH(P, C) k_gridder<P, C><<<g, b, 0, c->stream>>>(records, chunk_smax, (unsigned)nrb, (unsigned)nchan, c->grid, c->d_bank, c->prm.N, &c->d_acc->ticket, &c->d_acc->commits)
+    if (c->count_commits) {
+        switch (c->prm.npol) { case 1: IG_LAUNCH(1, true); break; case 2: IG_LAUNCH(2, true); break; default: IG_LAUNCH(4, true); break; }
+    } else {
+        switch (c->prm.npol) { case 1: IG_LAUNCH(1, false); break; case 2: IG_LAUNCH(2, false); break; default: IG_LAUNCH(4, false); break; }
     }
+#undef IG_LAUNCH
     IG_CUDA_OK(c, cudaGetLastError());
     return 1;
 }

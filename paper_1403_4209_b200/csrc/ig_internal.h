@@ -9,8 +9,15 @@
 #define IG_CH 128            // records per chunk (one work item per (row block, channel))
 #define IG_STAGE 32          // records per TMA stage
 #define IG_NSTAGE (IG_CH / IG_STAGE)
-#define IG_RMAX 8            // grid points per lane, at most
+#ifndef IG_RMAX
+#define IG_RMAX 5
+#endif
+// IG_RMAX: grid points per lane, at most (tunable with -DIG_RMAX for experiments)
 #define IG_TIMING_RING 64    // ig_grid calls whose event triples are kept
+#ifndef IG_GRID_CTAS_PER_SM
+#define IG_GRID_CTAS_PER_SM 4
+#endif
+// IG_GRID_CTAS_PER_SM: launch bound and persistent grid size
 #define IG_GRID_WARPS 4      // warps per gridder CTA
 
 // Device-side tail of the bank buffer: small tables and accumulators.
@@ -39,6 +46,7 @@ struct ig_ctx {
     char* bank_buf = nullptr; size_t bank_bytes = 0;
     cudaStream_t stream = nullptr;
     bool bound = false, have_bank = false;
+    bool count_commits = false;               // ig_set_commit_counting
     // bank description (host copies)
     std::vector<int> support;
     std::vector<uint32_t> koff;
@@ -60,15 +68,15 @@ static inline int ig_rec_stride(int npol) { return npol == 4 ? 48 : 32; }  // by
 void ig_taper_eval(const double* eta, int n, double* psi);
 
 // launchers (each returns the number of kernels launched, or -1 with ctx->err set)
-int ig_launch_sort_rows(ig_ctx* c, const int* baseline_id, long long nrow, uint32_t* perm_out,
-                        char* scratch, size_t scratch_bytes);
+int ig_launch_sort_rows(ig_ctx* c, const double* uvw, const int* baseline_id, long long nrow, double ref_freq_hz,
+                        uint32_t* perm_out, char* scratch, size_t scratch_bytes);
 size_t ig_sort_scratch_bytes(long long nrow);
 int ig_launch_index(ig_ctx* c, const double* uvw, const uint32_t* perm, long long nrow,
                     const double* d_freqs, int nchan, const float* vis, const float* wt,
                     char* records, uint32_t* chunk_smax);
 int ig_launch_debug_index(ig_ctx* c, const double* uvw, long long nrow, const double* d_freqs, int nchan,
                           int* X, int* Y, int* ou, int* ov, int* pl, int* fl);
-int ig_launch_gridder(ig_ctx* c, const char* records, const uint32_t* chunk_smax, long long n_chunks);
+int ig_launch_gridder(ig_ctx* c, const char* records, const uint32_t* chunk_smax, long long nrb, int nchan);
 int ig_launch_bank(ig_ctx* c, char* scratch, size_t scratch_bytes);
 size_t ig_bank_scratch_bytes(const ig_ctx* c);
 int ig_launch_zeta(ig_ctx* c);

@@ -55,7 +55,7 @@ extern "C" ig_status ig_measure_fp32_peak(void* cuda_stream, double* tflops) {
 // pixel) issued at pseudo-random pixels of a caller-provided buffer, nothing else in the loop. Gives the
 // L2 atomic ceiling (buffer resident in L2) and the HBM-backed ceiling (buffer far larger than L2) that
 // the byte side of the gridding roofline is compared with.
-__global__ void __launch_bounds__(256) k_red_rate(float* buf, unsigned long long n_pix, int iters, unsigned run_len) {
+__global__ void __launch_bounds__(256) k_red_rate(float* buf, unsigned long long n_pix, int iters, unsigned run_len, int planar) {
     unsigned long long x = 0x9E3779B97F4A7C15ull * (blockIdx.x * 256ull + threadIdx.x + 1);
     for (int it = 0; it < iters; ++it) {
         x ^= x << 13; x ^= x >> 7; x ^= x << 17;
@@ -63,14 +63,17 @@ __global__ void __launch_bounds__(256) k_red_rate(float* buf, unsigned long long
         // gridder's pattern (a warp commits a run of neighbouring pixels of one footprint row)
         unsigned long long start = __shfl_sync(0xffffffffu, x, 0) % n_pix;
         unsigned long long pix = (start + (threadIdx.x & 31) % run_len + ((threadIdx.x & 31) / run_len) * 4099ull) % n_pix;
-        float* g = buf + pix * 8;
+        float* g = planar ? buf + pix * 4 : buf + pix * 8;
+        float* g2 = planar ? g + n_pix * 4 : g + 4;      // planar: polarisation pairs in two planes
         asm volatile("red.global.add.v4.f32 [%0], {%1,%1,%1,%1};" ::"l"(g), "f"(1.0f) : "memory");
-        asm volatile("red.global.add.v4.f32 [%0], {%1,%1,%1,%1};" ::"l"(g + 4), "f"(1.0f) : "memory");
+        asm volatile("red.global.add.v4.f32 [%0], {%1,%1,%1,%1};" ::"l"(g2), "f"(1.0f) : "memory");
     }
 }
 
 extern "C" ig_status ig_measure_commit_rate(void* cuda_stream, void* buf_dev, size_t bytes, int run_len,
                                             double* gcommits_per_s) {
+    const int planar = run_len < 0;          // negative run length: planar polarisation-pair layout (experiment)
+    if (planar) run_len = -run_len;
     if (!buf_dev || bytes < 4096 || !gcommits_per_s || run_len < 1 || run_len > 32) return IG_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int dev = 0, sms = 0;
@@ -82,7 +85,7 @@ extern "C" ig_status ig_measure_commit_rate(void* cuda_stream, void* buf_dev, si
     double best = 0;
     for (int rep = 0; rep < 3; ++rep) {
         cudaEventRecord(e0, st);
-        k_red_rate<<<ctas, 256, 0, st>>>((float*)buf_dev, bytes / 32, iters, (unsigned)run_len);
+        k_red_rate<<<ctas, 256, 0, st>>>((float*)buf_dev, bytes / 32, iters, (unsigned)run_len, planar);
         cudaEventRecord(e1, st);
         if (cudaEventSynchronize(e1) != cudaSuccess) return IG_ECUDA;
         float ms = 0;

@@ -3,9 +3,16 @@
 // The thesis groups records by baseline with time ascending on the CPU (Alg 4.5,
 // PAPER.md:1613-1646) because the gridder accumulates along a baseline's track (:714).
 // Here the rows (nrow <= a few 1e7; records = rows x channels are never moved by the
-// sort) are ordered on the device: 4 passes of an 8-bit stable counting sort,
-// each = per-tile histogram -> exclusive scan -> stable scatter. Stability keeps the
-// input (time) order inside a baseline. Output: perm[j] = input row at sorted place j.
+// sort) are ordered on the device by the 48-bit key (uv tile in Morton order, baseline id):
+// 6 passes of an 8-bit stable counting sort, each = per-tile histogram -> exclusive scan
+// -> stable scatter. Stability keeps the input (time) order inside a (tile, baseline) run.
+// The tile part is new: rows whose footprints fall in the same 2-D region of the grid are
+// made neighbours in the work queue, so that the pixel commits of concurrently running
+// warps meet in the L2 instead of each costing an HBM read and write-back (profiles/
+// r01_v0_gridder.md: 1.0 TB of DRAM traffic on config 5 for 24 M touched pixels). A track
+// that crosses a tile edge is cut there, which costs one flush of the lane registers.
+// Output: perm[j] = input row at sorted place j.
+#include <stdlib.h>
 #include "ig_internal.h"
 
 #define SORT_THREADS 256
@@ -20,7 +27,7 @@ __device__ __forceinline__ uint32_t lanemask_lt() {
 }
 
 // per-warp digit counts of this CTA's tile into smem cnt[warp][256]
-__device__ __forceinline__ void tile_count(const uint32_t* __restrict__ keys, long long n, int shift,
+__device__ __forceinline__ void tile_count(const uint64_t* __restrict__ keys, long long n, int shift,
                                            uint32_t (*cnt)[256]) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     for (int i = threadIdx.x; i < SORT_WARPS * 256; i += SORT_THREADS) (&cnt[0][0])[i] = 0;
@@ -29,13 +36,13 @@ __device__ __forceinline__ void tile_count(const uint32_t* __restrict__ keys, lo
 #pragma unroll 4
     for (int s = 0; s < SORT_STEPS; ++s) {
         long long k = base + s * 32 + lane;
-        if (k < n) atomicAdd(&cnt[warp][(keys[k] >> shift) & 255u], 1u);
+        if (k < n) atomicAdd(&cnt[warp][(uint32_t)(keys[k] >> shift) & 255u], 1u);
     }
     __syncthreads();
 }
 
 __global__ void __launch_bounds__(SORT_THREADS)
-k_sort_hist(const uint32_t* __restrict__ keys, long long n, int shift, uint32_t* __restrict__ hist, int nblk) {
+k_sort_hist(const uint64_t* __restrict__ keys, long long n, int shift, uint32_t* __restrict__ hist, int nblk) {
     __shared__ uint32_t cnt[SORT_WARPS][256];
     tile_count(keys, n, shift, cnt);
     uint32_t t = 0;
@@ -89,8 +96,8 @@ __global__ void __launch_bounds__(1024) k_scan_excl(uint32_t* __restrict__ a, lo
 
 // vals_in == nullptr means the identity permutation (first pass)
 __global__ void __launch_bounds__(SORT_THREADS)
-k_sort_scatter(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals_in, long long n, int shift,
-               const uint32_t* __restrict__ hist, int nblk, uint32_t* __restrict__ keys_out,
+k_sort_scatter(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ vals_in, long long n, int shift,
+               const uint32_t* __restrict__ hist, int nblk, uint64_t* __restrict__ keys_out,
                uint32_t* __restrict__ vals_out) {
     __shared__ uint32_t cnt[SORT_WARPS][256];
     tile_count(keys, n, shift, cnt);
@@ -109,8 +116,8 @@ k_sort_scatter(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ v
     for (int s = 0; s < SORT_STEPS; ++s) {
         long long k = base + s * 32 + lane;
         bool act = k < n;
-        uint32_t key = act ? keys[k] : 0u;
-        uint32_t d = act ? ((key >> shift) & 255u) : 256u;
+        uint64_t key = act ? keys[k] : 0ull;
+        uint32_t d = act ? ((uint32_t)(key >> shift) & 255u) : 256u;
         uint32_t peers = __match_any_sync(0xffffffffu, d);
         uint32_t b = act ? cnt[warp][d] : 0u;
         __syncwarp();
@@ -124,30 +131,58 @@ k_sort_scatter(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ v
     }
 }
 
+// key = Morton(tile of the row's grid position at the reference frequency) << 32 | baseline id.
+// The position is the one the gridder uses (after the w<0 flip), in cells; it only steers the order.
+__device__ __forceinline__ uint32_t spread8(uint32_t x) {
+    x &= 0xffu;
+    x = (x | (x << 4)) & 0x0f0fu;
+    x = (x | (x << 2)) & 0x3333u;
+    x = (x | (x << 1)) & 0x5555u;
+    return x;
+}
+__global__ void k_sort_keys(const double* __restrict__ uvw, const int* __restrict__ baseline_id, long long n,
+                            double cells_per_m, int N, int tile_shift, uint64_t* __restrict__ keys) {
+    long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n) return;
+    double u = uvw[3 * r], v = uvw[3 * r + 1], w = uvw[3 * r + 2];
+    if (w < 0.0) { u = -u; v = -v; }
+    double fx = u * cells_per_m + 0.5 * N, fy = v * cells_per_m + 0.5 * N;
+    int x = (int)fmin(fmax(fx, 0.0), (double)(N - 1)), y = (int)fmin(fmax(fy, 0.0), (double)(N - 1));
+    uint32_t m = spread8((uint32_t)(x >> tile_shift)) | (spread8((uint32_t)(y >> tile_shift)) << 1);
+    keys[r] = ((uint64_t)m << 32) | (uint32_t)baseline_id[r];
+}
+
 size_t ig_sort_scratch_bytes(long long nrow) {
     long long nblk = (nrow + SORT_TILE - 1) / SORT_TILE;
     if (nblk < 1) nblk = 1;
-    // keysA, keysB, valsB (valsA is the caller's perm_out), hist
-    return 3 * ig_align((size_t)nrow * 4) + ig_align((size_t)nblk * 256 * 4);
+    // keysA, keysB (u64), valsB (valsA is the caller's perm_out), hist
+    return 2 * ig_align((size_t)nrow * 8) + ig_align((size_t)nrow * 4) + ig_align((size_t)nblk * 256 * 4);
 }
 
-int ig_launch_sort_rows(ig_ctx* c, const int* baseline_id, long long nrow, uint32_t* perm_out, char* scratch,
-                        size_t scratch_bytes) {
+int ig_launch_sort_rows(ig_ctx* c, const double* uvw, const int* baseline_id, long long nrow, double ref_freq_hz,
+                        uint32_t* perm_out, char* scratch, size_t scratch_bytes) {
     if (nrow >= (1ll << 32)) { c->err = "nrow must be < 2^32"; return -1; }
     if (scratch_bytes < ig_sort_scratch_bytes(nrow)) { c->err = "sort scratch too small"; return -1; }
     int nblk = (int)((nrow + SORT_TILE - 1) / SORT_TILE);
     if (nblk < 1) nblk = 1;
-    size_t a = ig_align((size_t)nrow * 4);
-    uint32_t* keysA = (uint32_t*)scratch;
-    uint32_t* keysB = (uint32_t*)(scratch + a);
-    uint32_t* valsB = (uint32_t*)(scratch + 2 * a);
-    uint32_t* hist = (uint32_t*)(scratch + 3 * a);
+    size_t a8 = ig_align((size_t)nrow * 8), a4 = ig_align((size_t)nrow * 4);
+    uint64_t* keysA = (uint64_t*)scratch;
+    uint64_t* keysB = (uint64_t*)(scratch + a8);
+    uint32_t* valsB = (uint32_t*)(scratch + 2 * a8);
+    uint32_t* hist = (uint32_t*)(scratch + 2 * a8 + a4);
     uint32_t* valsA = perm_out;
-    int launches = 0;
-    for (int pass = 0; pass < 4; ++pass) {
-        const uint32_t* kin = pass == 0 ? (const uint32_t*)baseline_id : ((pass & 1) ? keysB : keysA);
+    // tiles of 2^tile_shift cells, at most 256 per axis, at least 128 cells wide
+    int tile_shift = 7;
+    while ((c->prm.N >> tile_shift) > 256) ++tile_shift;
+    if (const char* e = getenv("IG_TILE_SHIFT")) { int t = atoi(e); if (t >= tile_shift && t <= 15) tile_shift = t; }
+    const double cells_per_m = ref_freq_hz * c->prm.ku / (double)c->prm.beta;
+    k_sort_keys<<<(unsigned)((nrow + 255) / 256), 256, 0, c->stream>>>(uvw, baseline_id, nrow, cells_per_m, c->prm.N,
+                                                                      tile_shift, keysA);
+    int launches = 1;
+    for (int pass = 0; pass < 6; ++pass) {     // bytes 0-3 baseline id, bytes 4-5 Morton tile
+        const uint64_t* kin = (pass & 1) ? keysB : keysA;
         const uint32_t* vin = pass == 0 ? nullptr : ((pass & 1) ? valsB : valsA);
-        uint32_t* kout = (pass & 1) ? keysA : keysB;
+        uint64_t* kout = (pass & 1) ? keysA : keysB;
         uint32_t* vout = (pass & 1) ? valsA : valsB;
         k_sort_hist<<<nblk, SORT_THREADS, 0, c->stream>>>(kin, nrow, pass * 8, hist, nblk);
         k_scan_excl<<<1, 1024, 0, c->stream>>>(hist, (long long)nblk * 256);
@@ -155,5 +190,5 @@ int ig_launch_sort_rows(ig_ctx* c, const int* baseline_id, long long nrow, uint3
         launches += 3;
     }
     IG_CUDA_OK(c, cudaGetLastError());
-    return launches;   // result is in valsA == perm_out after the 4th pass
+    return launches;   // result is in valsA == perm_out after the 6th pass
 }
