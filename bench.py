@@ -223,9 +223,7 @@ def run_ours(args):
     gridded, dropped, updates = g.stats()
     commits = g.commits()
     g.set_commit_counting(False)
-    touched = int(torch.count_nonzero(g.grid.view(cfg.grid_n * cfg.grid_n, -1).abs().sum(dim=1)).item()) \
-        if cfg.grid_n <= 8192 else int(sum(torch.count_nonzero(c.view(-1, npol * 2).abs().sum(dim=1)).item()
-                                           for c in g.grid.view(-1, npol, 2).chunk(16)))
+    touched = g.touched_pixels()
     launches_per_step = g.last_launches()
     for _ in range(max(0, args.warmup - 1)):
         step()

@@ -56,8 +56,10 @@ ig_status ig_create(ig_ctx** out, int grid_n, double cell_rad, int n_wplanes, in
 void ig_destroy(ig_ctx* ctx);
 const char* ig_last_error(const ig_ctx* ctx);
 
-/* Bytes of the uv-grid: N*N*n_pol complex64, layout [y][x][pol][re,im]
- * ("multi-polarised pixel", :1319; reading 13). Pixel (N/2,N/2) is u=v=0. */
+/* Bytes of the uv-grid: N*N*n_pol complex64. Layout (reading 13): n_pol 1 or 2: [y][x][pol][re,im]
+ * ("multi-polarised pixel", :1319); n_pol 4: two planes of polarisation pairs, [pair][y][x][2][re,im]
+ * with pol = 2*pair + k, so that a pixel commit is two 16-byte vector reductions and neighbouring
+ * pixels share L2 sectors. Pixel (N/2,N/2) is u=v=0. */
 size_t ig_grid_bytes(const ig_ctx* ctx);
 /* Bytes of work_dev that one ig_grid call of (nrow, nchan) needs. */
 size_t ig_workspace_bytes(const ig_ctx* ctx, long long nrow, int nchan);

@@ -237,9 +237,23 @@ class Gridder:
         return dict(zip(("X", "Y", "off_u", "off_v", "plane", "flags"), [o.cpu().numpy() for o in outs]))
 
     def grid_complex(self) -> np.ndarray:
-        """The grid as complex64 numpy [N][N][npol] (synchronises)."""
+        """The grid as complex64 numpy [N][N][npol] (synchronises); undoes the 4-pol pair-plane layout."""
         self.torch.cuda.synchronize(self.device)
-        return self.grid.cpu().numpy().view(np.complex64)[..., 0]
+        g = self.grid
+        if self.n_pol == 4:
+            n = self.grid_n
+            g = g.view(2, n, n, 2, 2).permute(1, 2, 0, 3, 4).reshape(n, n, 4, 2)
+        return g.contiguous().cpu().numpy().view(np.complex64)[..., 0]
+
+    def touched_pixels(self) -> int:
+        """Pixels with a non-zero value in any polarisation (synchronises)."""
+        t, n = self.torch, self.grid_n
+        g = self.grid.view(2, n * n, 4) if self.n_pol == 4 else self.grid.view(1, n * n, self.n_pol * 2)
+        hit = t.zeros(n * n, dtype=t.bool, device=self.device)
+        for part in g:
+            for lo in range(0, n * n, 1 << 26):
+                hit[lo:lo + (1 << 26)] |= (part[lo:lo + (1 << 26)] != 0).any(dim=1)
+        return int(hit.sum().item())
 
     def close(self):
         if self.ctx:

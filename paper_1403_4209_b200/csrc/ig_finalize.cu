@@ -14,7 +14,10 @@ __global__ void k_fin_extract(const float2* __restrict__ grid, float2* __restric
     int x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y;
     if (x >= N) return;
     int sx = (x + N / 2) % N, sy = (y + N / 2) % N;      // ifftshift: origin N/2 -> 0
-    plane[(size_t)y * N + x] = grid[((size_t)sy * N + sx) * NPOL + pol];
+    // 4 pol: two planes of polarisation pairs [pair][y][x][2]; 1 or 2 pol: [y][x][pol]
+    constexpr int PP = NPOL == 4 ? 2 : NPOL;
+    const size_t base = NPOL == 4 ? (size_t)(pol >> 1) * N * N * 2 : 0;
+    plane[(size_t)y * N + x] = grid[base + ((size_t)sy * N + sx) * PP + (NPOL == 4 ? (pol & 1) : pol)];
 }
 
 __global__ void k_fin_write(const float2* __restrict__ plane, float* __restrict__ image, const double* __restrict__ corr,

@@ -16,8 +16,10 @@
 //    mbarrier), IG_NSTAGE stages in flight per warp; the record header and visibility are
 //    then shared-memory broadcasts;
 //  - support changes inside a chunk need no flush logic: a lane's point simply changes;
-//  - commits are vector reductions, red.global.add.v4.f32: one 4-pol pixel = 2 instructions,
-//    one 32-byte L2 sector.
+//  - commits are vector reductions, red.global.add.v4.f32. The 4-pol grid is stored as two planes of
+//    polarisation pairs, so a pixel commit is 2 instructions of 16 bytes and NEIGHBOURING lanes (consecutive
+//    x) share a 32-byte sector: half the L2 atomic sector operations of a pixel-interleaved layout
+//    (measured 174 vs 110 G pixel commits/s, ig_measure_commit_rate).
 // Kernel values come straight from the bank with read-only loads: each (record, tap) value
 // is used once per record, so the only reuse is across records and that lives in L1/L2.
 #include "ig_internal.h"
@@ -56,22 +58,23 @@ __device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t
 // and no BSSY/BSYNC pair is issued. COUNT adds the commit counter (ig_get_commits).
 template <int NPOL, bool COUNT>
 __device__ __forceinline__ void commit_step(float (&a)[2 * NPOL], int& prev, int pix, float* __restrict__ grid,
-                                            unsigned& n_commit) {
+                                            unsigned long long plane_bytes, unsigned& n_commit) {
     if constexpr (COUNT) n_commit += (pix != prev && prev >= 0) ? 1u : 0u;
     if constexpr (NPOL == 4) {
         asm volatile(
             "{\n\t.reg .pred p, q;\n\t.reg .u64 ad;\n\t"
             "setp.ne.s32 p, %9, %8;\n\t"
             "setp.ge.and.s32 q, %8, 0, p;\n\t"
-            "@q mad.wide.s32 ad, %8, 32, %10;\n\t"
+            "@q mad.wide.s32 ad, %8, 16, %10;\n\t"
             "@q red.global.add.v4.f32 [ad], {%0,%1,%2,%3};\n\t"
-            "@q red.global.add.v4.f32 [ad+16], {%4,%5,%6,%7};\n\t"
+            "@q add.u64 ad, ad, %11;\n\t"
+            "@q red.global.add.v4.f32 [ad], {%4,%5,%6,%7};\n\t"
             "@p mov.f32 %0, 0f00000000;\n\t@p mov.f32 %1, 0f00000000;\n\t@p mov.f32 %2, 0f00000000;\n\t"
             "@p mov.f32 %3, 0f00000000;\n\t@p mov.f32 %4, 0f00000000;\n\t@p mov.f32 %5, 0f00000000;\n\t"
             "@p mov.f32 %6, 0f00000000;\n\t@p mov.f32 %7, 0f00000000;\n\t"
             "@p mov.s32 %8, %9;\n\t}"
             : "+f"(a[0]), "+f"(a[1]), "+f"(a[2]), "+f"(a[3]), "+f"(a[4]), "+f"(a[5]), "+f"(a[6]), "+f"(a[7]), "+r"(prev)
-            : "r"(pix), "l"(grid));
+            : "r"(pix), "l"(grid), "l"(plane_bytes));
     } else if constexpr (NPOL == 2) {
         asm volatile(
             "{\n\t.reg .pred p, q;\n\t.reg .u64 ad;\n\t"
@@ -100,14 +103,17 @@ __device__ __forceinline__ void commit_step(float (&a)[2 * NPOL], int& prev, int
 
 // final flush of one point
 template <int NPOL>
-__device__ __forceinline__ void commit(float* __restrict__ grid, int pix, float (&a)[2 * NPOL]) {
-    float* g = grid + (size_t)pix * (2 * NPOL);
+__device__ __forceinline__ void commit(float* __restrict__ grid, unsigned long long plane_bytes, int pix, float (&a)[2 * NPOL]) {
     if constexpr (NPOL == 1) {
+        float* g = grid + (size_t)pix * 2;
         asm volatile("red.global.add.v2.f32 [%0], {%1,%2};" ::"l"(g), "f"(a[0]), "f"(a[1]) : "memory");
     } else {
+        float* g = grid + (size_t)pix * 4;       // one plane holds a polarisation pair per pixel
         asm volatile("red.global.add.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(g), "f"(a[0]), "f"(a[1]), "f"(a[2]), "f"(a[3]) : "memory");
-        if constexpr (NPOL == 4)
-            asm volatile("red.global.add.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(g + 4), "f"(a[4]), "f"(a[5]), "f"(a[6]), "f"(a[7]) : "memory");
+        if constexpr (NPOL == 4) {
+            float* g2 = reinterpret_cast<float*>(reinterpret_cast<char*>(g) + plane_bytes);
+            asm volatile("red.global.add.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(g2), "f"(a[4]), "f"(a[5]), "f"(a[6]), "f"(a[7]) : "memory");
+        }
     }
 }
 
@@ -119,6 +125,7 @@ template <int NPOL, int R, bool COUNT>
 __device__ __forceinline__ unsigned grid_run(const char* __restrict__ rp, int n_rec, int S, int q0,
                                              float* __restrict__ grid, const float2* __restrict__ bank, int N) {
     constexpr int STRIDE = NPOL == 4 ? 48 : 32;
+    const unsigned long long plane_bytes = (unsigned long long)N * N * 16;   // 4 pol: two planes of pol pairs
     float acc[R][2 * NPOL];
     int prev[R], ii[R], jj[R];
     uint32_t amask = 0;
@@ -161,7 +168,7 @@ __device__ __forceinline__ unsigned grid_run(const char* __restrict__ rp, int n_
         }
 #pragma unroll
         for (int k = 0; k < R; ++k) {
-            commit_step<NPOL, COUNT>(acc[k], prev[k], pix[k], grid, n_commit);
+            commit_step<NPOL, COUNT>(acc[k], prev[k], pix[k], grid, plane_bytes, n_commit);
 #pragma unroll
             for (int q = 0; q < NPOL; ++q) {
                 acc[k][2 * q] = fmaf(v[2 * q], kv[k].x, acc[k][2 * q]);
@@ -173,7 +180,7 @@ __device__ __forceinline__ unsigned grid_run(const char* __restrict__ rp, int n_
     }
 #pragma unroll
     for (int k = 0; k < R; ++k)
-        if (prev[k] >= 0) { commit<NPOL>(grid, prev[k], acc[k]); ++n_commit; }
+        if (prev[k] >= 0) { commit<NPOL>(grid, plane_bytes, prev[k], acc[k]); ++n_commit; }
     return n_commit;
 }
 
