@@ -51,59 +51,79 @@ __device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t
                  : "memory");
 }
 
+// Packed fp32 pairs (sm_100a FFMA2, PTX fma.rn.f32x2): one complex accumulator = one 64-bit register
+// pair (re, im); a complex multiply-accumulate acc += v * k is exactly two FFMA2
+//   (re,im) += (v_re, v_re) * (k_re, k_im);   (re,im) += (-v_im, v_im) * (k_im, k_re)
+// - ptxas folds the broadcast, the swap and the half negation into operand modifiers (.F32, .LO_HI, .NP).
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ void cmac(f32x2& acc, float v_re, float v_im, f32x2 k) {
+    float k_re, k_im;
+    unpack2(k, k_re, k_im);
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(pack2(v_re, v_re)), "l"(k));
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(pack2(-v_im, v_im)), "l"(pack2(k_im, k_re)));
+}
+
 // Commit step of one owned point, branch-free: if the record's pixel differs from the one the lane
 // holds, the held sums go to the grid with vector reductions (unless the lane held nothing, prev < 0),
 // the sums restart from zero and the lane takes the new pixel. Written as predicated PTX so that the
-// sums stay in place (the compiler's own if-conversion copied all eight registers per point and record)
-// and no BSSY/BSYNC pair is issued. COUNT adds the commit counter (ig_get_commits).
+// sums stay in place. COUNT adds the commit counter (ig_get_commits).
 template <int NPOL, bool COUNT>
-__device__ __forceinline__ void commit_step(float (&a)[2 * NPOL], int& prev, int pix, float* __restrict__ grid,
+__device__ __forceinline__ void commit_step(f32x2 (&a)[NPOL], int& prev, int pix, float* __restrict__ grid,
                                             unsigned long long plane_bytes, unsigned& n_commit) {
     if constexpr (COUNT) n_commit += (pix != prev && prev >= 0) ? 1u : 0u;
     if constexpr (NPOL == 4) {
         asm volatile(
-            "{\n\t.reg .pred p, q;\n\t.reg .u64 ad;\n\t"
-            "setp.ne.s32 p, %9, %8;\n\t"
-            "setp.ge.and.s32 q, %8, 0, p;\n\t"
-            "@q mad.wide.s32 ad, %8, 16, %10;\n\t"
-            "@q red.global.add.v4.f32 [ad], {%0,%1,%2,%3};\n\t"
-            "@q add.u64 ad, ad, %11;\n\t"
-            "@q red.global.add.v4.f32 [ad], {%4,%5,%6,%7};\n\t"
-            "@p mov.f32 %0, 0f00000000;\n\t@p mov.f32 %1, 0f00000000;\n\t@p mov.f32 %2, 0f00000000;\n\t"
-            "@p mov.f32 %3, 0f00000000;\n\t@p mov.f32 %4, 0f00000000;\n\t@p mov.f32 %5, 0f00000000;\n\t"
-            "@p mov.f32 %6, 0f00000000;\n\t@p mov.f32 %7, 0f00000000;\n\t"
-            "@p mov.s32 %8, %9;\n\t}"
-            : "+f"(a[0]), "+f"(a[1]), "+f"(a[2]), "+f"(a[3]), "+f"(a[4]), "+f"(a[5]), "+f"(a[6]), "+f"(a[7]), "+r"(prev)
+            "{\n\t.reg .pred p, q;\n\t.reg .u64 ad;\n\t.reg .f32 f<8>;\n\t"
+            "setp.ne.s32 p, %5, %4;\n\t"
+            "setp.ge.and.s32 q, %4, 0, p;\n\t"
+            "mov.b64 {f0,f1}, %0;\n\tmov.b64 {f2,f3}, %1;\n\tmov.b64 {f4,f5}, %2;\n\tmov.b64 {f6,f7}, %3;\n\t"
+            "@q mad.wide.s32 ad, %4, 16, %6;\n\t"
+            "@q red.global.add.v4.f32 [ad], {f0,f1,f2,f3};\n\t"
+            "@q add.u64 ad, ad, %7;\n\t"
+            "@q red.global.add.v4.f32 [ad], {f4,f5,f6,f7};\n\t"
+            "@p mov.b64 %0, 0;\n\t@p mov.b64 %1, 0;\n\t@p mov.b64 %2, 0;\n\t@p mov.b64 %3, 0;\n\t"
+            "@p mov.s32 %4, %5;\n\t}"
+            : "+l"(a[0]), "+l"(a[1]), "+l"(a[2]), "+l"(a[3]), "+r"(prev)
             : "r"(pix), "l"(grid), "l"(plane_bytes));
     } else if constexpr (NPOL == 2) {
         asm volatile(
-            "{\n\t.reg .pred p, q;\n\t.reg .u64 ad;\n\t"
-            "setp.ne.s32 p, %5, %4;\n\t"
-            "setp.ge.and.s32 q, %4, 0, p;\n\t"
-            "@q mad.wide.s32 ad, %4, 16, %6;\n\t"
-            "@q red.global.add.v4.f32 [ad], {%0,%1,%2,%3};\n\t"
-            "@p mov.f32 %0, 0f00000000;\n\t@p mov.f32 %1, 0f00000000;\n\t@p mov.f32 %2, 0f00000000;\n\t"
-            "@p mov.f32 %3, 0f00000000;\n\t"
-            "@p mov.s32 %4, %5;\n\t}"
-            : "+f"(a[0]), "+f"(a[1]), "+f"(a[2]), "+f"(a[3]), "+r"(prev)
+            "{\n\t.reg .pred p, q;\n\t.reg .u64 ad;\n\t.reg .f32 f<4>;\n\t"
+            "setp.ne.s32 p, %3, %2;\n\t"
+            "setp.ge.and.s32 q, %2, 0, p;\n\t"
+            "mov.b64 {f0,f1}, %0;\n\tmov.b64 {f2,f3}, %1;\n\t"
+            "@q mad.wide.s32 ad, %2, 16, %4;\n\t"
+            "@q red.global.add.v4.f32 [ad], {f0,f1,f2,f3};\n\t"
+            "@p mov.b64 %0, 0;\n\t@p mov.b64 %1, 0;\n\t"
+            "@p mov.s32 %2, %3;\n\t}"
+            : "+l"(a[0]), "+l"(a[1]), "+r"(prev)
             : "r"(pix), "l"(grid));
     } else {
         asm volatile(
-            "{\n\t.reg .pred p, q;\n\t.reg .u64 ad;\n\t"
-            "setp.ne.s32 p, %3, %2;\n\t"
-            "setp.ge.and.s32 q, %2, 0, p;\n\t"
-            "@q mad.wide.s32 ad, %2, 8, %4;\n\t"
-            "@q red.global.add.v2.f32 [ad], {%0,%1};\n\t"
-            "@p mov.f32 %0, 0f00000000;\n\t@p mov.f32 %1, 0f00000000;\n\t"
-            "@p mov.s32 %2, %3;\n\t}"
-            : "+f"(a[0]), "+f"(a[1]), "+r"(prev)
+            "{\n\t.reg .pred p, q;\n\t.reg .u64 ad;\n\t.reg .f32 f<2>;\n\t"
+            "setp.ne.s32 p, %2, %1;\n\t"
+            "setp.ge.and.s32 q, %1, 0, p;\n\t"
+            "mov.b64 {f0,f1}, %0;\n\t"
+            "@q mad.wide.s32 ad, %1, 8, %3;\n\t"
+            "@q red.global.add.v2.f32 [ad], {f0,f1};\n\t"
+            "@p mov.b64 %0, 0;\n\t"
+            "@p mov.s32 %1, %2;\n\t}"
+            : "+l"(a[0]), "+r"(prev)
             : "r"(pix), "l"(grid));
     }
 }
 
 // final flush of one point
 template <int NPOL>
-__device__ __forceinline__ void commit(float* __restrict__ grid, unsigned long long plane_bytes, int pix, float (&a)[2 * NPOL]) {
+__device__ __forceinline__ void commit(float* __restrict__ grid, unsigned long long plane_bytes, int pix, f32x2 (&acc)[NPOL]) {
+    float a[2 * NPOL];
+#pragma unroll
+    for (int q = 0; q < NPOL; ++q) unpack2(acc[q], a[2 * q], a[2 * q + 1]);
     if constexpr (NPOL == 1) {
         float* g = grid + (size_t)pix * 2;
         asm volatile("red.global.add.v2.f32 [%0], {%1,%2};" ::"l"(g), "f"(a[0]), "f"(a[1]) : "memory");
@@ -126,7 +146,7 @@ __device__ __forceinline__ unsigned grid_run(const char* __restrict__ rp, int n_
                                              float* __restrict__ grid, const float2* __restrict__ bank, int N) {
     constexpr int STRIDE = NPOL == 4 ? 48 : 32;
     const unsigned long long plane_bytes = (unsigned long long)N * N * 16;   // 4 pol: two planes of pol pairs
-    float acc[R][2 * NPOL];
+    f32x2 acc[R][NPOL];
     int prev[R], ii[R], jj[R];
     uint32_t amask = 0;
 #pragma unroll
@@ -139,13 +159,17 @@ __device__ __forceinline__ unsigned grid_run(const char* __restrict__ rp, int n_
         amask |= act ? (1u << k) : 0u;
         prev[k] = -1;
 #pragma unroll
-        for (int e = 0; e < 2 * NPOL; ++e) acc[k][e] = 0.f;
+        for (int e = 0; e < NPOL; ++e) acc[k][e] = 0ull;
     }
+    const unsigned long long* __restrict__ bank64 = reinterpret_cast<const unsigned long long*>(bank);
     unsigned n_commit = 0;
+    uint32_t krel[R];                  // tap index ty*S+tx of each point for the current window position
+#pragma unroll
+    for (int k = 0; k < R; ++k) krel[k] = 0;
+    uint32_t last_x = 0xffffffffu, last_z = 0xffffffffu;
 #pragma unroll 1
     for (int r = 0; r < n_rec; ++r, rp += STRIDE) {
         const uint4 h = *reinterpret_cast<const uint4*>(rp);
-        const int cm = (int)(h.z & 0xffu), dm = (int)((h.z >> 8) & 0xffu);
         float v[2 * NPOL];
         {
             const float4 a = *reinterpret_cast<const float4*>(rp + 16);
@@ -156,26 +180,34 @@ __device__ __forceinline__ unsigned grid_run(const char* __restrict__ rp, int n_
                 v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
             }
         }
-        float2 kv[R];
-        int pix[R];
+        f32x2 kv[R];
+        // Same window as the record before (same cell; only the sub-cell offsets, hence the kernel matrix,
+        // may differ): every lane keeps its pixels and taps, so the index arithmetic and the commit test
+        // are skipped. Slow baselines stay in a cell for many records (warp-uniform branch).
+        const bool same = (h.x == last_x) && ((h.z & 0x00ffffffu) == last_z);
+        if (same) {
 #pragma unroll
-        for (int k = 0; k < R; ++k) {
-            const int tu = ii[k] + cm, tv = jj[k] + dm;
-            const int tx = (int)min((unsigned)tu, (unsigned)(tu - S));     // (i + c) mod S
-            const int ty = (int)min((unsigned)tv, (unsigned)(tv - S));
-            pix[k] = (amask & (1u << k)) ? ty * N + ((int)h.x + tx) : -1;
-            kv[k] = __ldg(bank + (uint32_t)(ty * S + (tx + (int)h.y)));   // 32-bit element index
+            for (int k = 0; k < R; ++k) kv[k] = __ldg(bank64 + (uint32_t)(krel[k] + h.y));
+        } else {
+            last_x = h.x; last_z = h.z & 0x00ffffffu;
+            const int cm = (int)(h.z & 0xffu), dm = (int)((h.z >> 8) & 0xffu);
+            int pix[R];
+#pragma unroll
+            for (int k = 0; k < R; ++k) {
+                const int tu = ii[k] + cm, tv = jj[k] + dm;
+                const int tx = (int)min((unsigned)tu, (unsigned)(tu - S));     // (i + c) mod S
+                const int ty = (int)min((unsigned)tv, (unsigned)(tv - S));
+                pix[k] = (amask & (1u << k)) ? ty * N + ((int)h.x + tx) : -1;
+                krel[k] = (uint32_t)(ty * S + tx);
+                kv[k] = __ldg(bank64 + (uint32_t)(krel[k] + h.y));            // 32-bit element index
+            }
+#pragma unroll
+            for (int k = 0; k < R; ++k) commit_step<NPOL, COUNT>(acc[k], prev[k], pix[k], grid, plane_bytes, n_commit);
         }
 #pragma unroll
         for (int k = 0; k < R; ++k) {
-            commit_step<NPOL, COUNT>(acc[k], prev[k], pix[k], grid, plane_bytes, n_commit);
 #pragma unroll
-            for (int q = 0; q < NPOL; ++q) {
-                acc[k][2 * q] = fmaf(v[2 * q], kv[k].x, acc[k][2 * q]);
-                acc[k][2 * q] = fmaf(-v[2 * q + 1], kv[k].y, acc[k][2 * q]);
-                acc[k][2 * q + 1] = fmaf(v[2 * q], kv[k].y, acc[k][2 * q + 1]);
-                acc[k][2 * q + 1] = fmaf(v[2 * q + 1], kv[k].x, acc[k][2 * q + 1]);
-            }
+            for (int q = 0; q < NPOL; ++q) cmac(acc[k][q], v[2 * q], v[2 * q + 1], kv[k]);
         }
     }
 #pragma unroll

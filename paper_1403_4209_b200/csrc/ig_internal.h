@@ -10,7 +10,7 @@
 #define IG_STAGE 32          // records per TMA stage
 #define IG_NSTAGE (IG_CH / IG_STAGE)
 #ifndef IG_RMAX
-#define IG_RMAX 5
+#define IG_RMAX 4
 #endif
 // IG_RMAX: grid points per lane, at most (tunable with -DIG_RMAX for experiments)
 #define IG_TIMING_RING 64    // ig_grid calls whose event triples are kept
