@@ -36,6 +36,8 @@ SIGNATURES = {
     "ig_finalize": (_i, [_vp, _vp, _vp]),
     "ig_get_stats": (_i, [_vp, C.POINTER(_ll), C.POINTER(_ll), C.POINTER(_ll)]),
     "ig_get_commits": (_i, [_vp, C.POINTER(_ll)]),
+    "ig_set_compression": (_i, [_vp, _i]),
+    "ig_get_compressed": (_i, [_vp, C.POINTER(_ll)]),
     "ig_set_commit_counting": (_i, [_vp, _i]),
     "ig_measure_fp32_peak": (_i, [_vp, C.POINTER(_d)]),
     "ig_measure_commit_rate": (_i, [_vp, _vp, _sz, _i, C.POINTER(_d)]),
@@ -192,6 +194,14 @@ class Gridder:
         g, d, u = _ll(), _ll(), _ll()
         self._check(self.lib.ig_get_stats(self.ctx, C.byref(g), C.byref(d), C.byref(u)), "ig_get_stats")
         return g.value, d.value, u.value
+
+    def set_compression(self, on: bool):
+        self._check(self.lib.ig_set_compression(self.ctx, int(bool(on))), "ig_set_compression")
+
+    def compressed(self) -> int:
+        n = _ll()
+        self._check(self.lib.ig_get_compressed(self.ctx, C.byref(n)), "ig_get_compressed")
+        return n.value
 
     def set_commit_counting(self, on: bool):
         self._check(self.lib.ig_set_commit_counting(self.ctx, int(bool(on))), "ig_set_commit_counting")

@@ -273,6 +273,23 @@ ig_status ig_set_commit_counting(ig_ctx* c, int on) {
     return IG_OK;
 }
 
+ig_status ig_set_compression(ig_ctx* c, int on) {
+    if (!c) return IG_EINVAL;
+    c->compress = on != 0;
+    return IG_OK;
+}
+
+ig_status ig_get_compressed(ig_ctx* c, long long* n) {
+    if (!c || !n) return IG_EINVAL;
+    if (!c->bound) return fail(c, IG_ESTATE, "ig_bind first");
+    IgAccum a;
+    if (cudaMemcpyAsync(&a, c->d_acc, sizeof(a), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess)
+        return fail(c, IG_ECUDA, std::string("ig_get_compressed: ") + cudaGetErrorString(cudaGetLastError()));
+    *n = (long long)a.merged;
+    return IG_OK;
+}
+
 ig_status ig_get_commits(ig_ctx* c, long long* n) {
     if (!c || !n) return IG_EINVAL;
     if (!c->bound) return fail(c, IG_ESTATE, "ig_bind first");

@@ -25,6 +25,7 @@ struct IgPlaneEntry { int support; uint32_t koff; };   // koff in complex elemen
 struct IgAccum {
     double norm[4];                     // eq 4.5 normaliser per polarisation
     unsigned long long gridded, dropped, updates;   // eq 4.17
+    unsigned long long merged;          // records pre-summed into their predecessor (compression)
     unsigned long long commits;         // pixel commits (atomic reductions of one multi-pol pixel) by the gridder
     unsigned int ticket;                // work queue of the gridder
     unsigned int max_key;               // largest baseline id of the current call
@@ -46,6 +47,7 @@ struct ig_ctx {
     char* bank_buf = nullptr; size_t bank_bytes = 0;
     cudaStream_t stream = nullptr;
     bool bound = false, have_bank = false;
+    bool compress = true;                     // ig_set_compression
     bool count_commits = false;               // ig_set_commit_counting
     // bank description (host copies)
     std::vector<int> support;

@@ -229,3 +229,58 @@ def test_errors_are_statuses(torch_cuda):
     g = Gridder(256, 1e-4, 1, 8, 7, 1)
     with pytest.raises(IgError):
         g.stats()                               # not bound yet
+
+
+def test_full_size_config2_whole_grid(orc, torch_cuda):
+    """BASELINE.json configs[1] at FULL size (8.26 M records, 1024^2 x 4 pol), whole grid element by element,
+    in the launch configuration bench.py times (same entry point, same persistent grid)."""
+    cfg = synth.CONFIGS[1]
+    wl = synth.make_workload(cfg)
+    ref = oracle_run(orc, wl)
+    g = make_gridder(wl)
+    g.build_wkernels(wl["w_max"])
+    uvw, bl, vis, wt = to_dev(torch_cuda, wl)
+    g.set_commit_counting(True)
+    g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+    frob, mx = check_grid(g.grid_complex(), ref["grid"])
+    assert g.stats() == tuple(int(x) for x in ref["stats"])
+    assert g.commits() > 0
+    # counting off (the timed configuration) gives the same grid up to summation order
+    g.reset()
+    g.set_commit_counting(False)
+    g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+    check_grid(g.grid_complex(), ref["grid"])
+    assert g.touched_pixels() == int((np.abs(ref["grid"]).sum(axis=2) != 0).sum())
+
+
+def test_compression_same_grid_and_counts(orc, torch_cuda):
+    """Compression (:1295-1305): rows repeated in time are summed before gridding; same grid as the oracle
+    (which grids every record), with and without compression; the merged-record counter sees them."""
+    cfg = small(synth.CONFIGS[1], n_station=9, n_time=90, n_chan=3, n_wplanes=8)
+    wl = synth.make_workload(cfg)
+    n_bl = 9 * 8 // 2
+    rep = 3                                            # every time step appears three times in a row
+    def tile(a):
+        a = a.reshape((cfg.n_time, n_bl) + a.shape[1:])
+        return np.ascontiguousarray(np.repeat(a, rep, axis=0).reshape((-1,) + a.shape[2:]))
+    rng = np.random.default_rng(3)
+    wl = dict(wl, uvw_m=tile(wl["uvw_m"]), baseline=tile(wl["baseline"]))
+    shape = (wl["uvw_m"].shape[0], cfg.n_chan, cfg.n_pol)
+    wl["vis"] = (rng.standard_normal(shape) + 1j * rng.standard_normal(shape)).astype(np.complex64)
+    wl["weights"] = rng.uniform(0.5, 1.0, shape).astype(np.float32)
+    ref = oracle_run(orc, wl)
+    uvw, bl, vis, wt = to_dev(torch_cuda, wl)
+    merged = {}
+    for on in (True, False):
+        g = make_gridder(wl)
+        g.debug_set_wkernels(wl["w_max"], ref["bank"].astype(np.complex64))
+        g.set_compression(on)
+        g.set_commit_counting(True)
+        g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+        check_grid(g.grid_complex(), ref["grid"])
+        assert g.stats() == tuple(int(x) for x in ref["stats"])     # eq 4.17 counts every gridded record
+        merged[on] = g.compressed()
+    nrec = shape[0] * cfg.n_chan
+    assert merged[False] == 0
+    # two of every three records are merged, except where a 128-row work item or a tile edge cuts a triple
+    assert 0.6 * nrec <= merged[True] <= (2 * nrec) // 3
