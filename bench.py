@@ -39,6 +39,7 @@ def parse():
     ap.add_argument("--config", type=int, default=int(os.environ.get("IG_BENCH_CONFIG", "5")),
                     help="BASELINE.json configuration 1..5 (default 5, the largest W-projection config the target is quoted on)")
     ap.add_argument("--support-law", default="w", choices=["w", "k"])
+    ap.add_argument("--no-compress", action="store_true", help="switch compression off (thesis: real vs total rate)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU time of the oracle sample")
@@ -201,6 +202,7 @@ def run_ours(args):
     torch.cuda.synchronize(dev)
     t_bank = time.perf_counter() - t0
     fp32_peak = g.measure_fp32_peak()
+    g.set_compression(not args.no_compress)
 
     pin = (lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()) if not args.no_e2e else None
     vis_f = np.ascontiguousarray(wl["vis"]).view(np.float32).reshape(nrow, nchan, npol, 2)
@@ -222,6 +224,7 @@ def run_ours(args):
     step()
     gridded, dropped, updates = g.stats()
     commits = g.commits()
+    compressed = g.compressed()
     g.set_commit_counting(False)
     touched = g.touched_pixels()
     launches_per_step = g.last_launches()
@@ -303,6 +306,9 @@ def run_ours(args):
                    "l2": "inputs (%.1f GB) larger than L2; no flush needed" % (h2d_bytes / 1e9)},
         "visibilities_per_s": world * gridded / (ms_step * 1e-3),
         "records_gridded": gridded, "records_dropped": dropped, "updates_per_step": updates,
+        "compression": {"enabled": not args.no_compress, "records_compressed": compressed,
+                        "note": "value counts every gridded record (thesis total rate, PAPER.md:1767); "
+                                "real rate = value * (1 - records_compressed / records_gridded)"},
         "ingest_ms": ingest_ms, "gridder_ms": gridder_ms, "gridder_updates_per_s": updates / gs,
         "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
         "clocks": clocks, "setup": {"generate_s": t_gen, "build_wkernels_s": t_bank},

@@ -132,7 +132,7 @@ ig_status ig_get_stats(ig_ctx* ctx, long long* n_gridded, long long* n_dropped, 
 /* Compression (eq 4.9 :1407-1414): consecutive records of a work item with the same cell,
  * w-plane and sub-cell offsets are summed before gridding. On by default; the grid is the same up to rounding.
  * eq 4.17's update count keeps counting every gridded record (the thesis's "total" rate, :1767).
- * ig_get_compressed: records merged into their predecessor so far, counted only while commit counting is on. */
+ * ig_get_compressed: records merged into their predecessor so far. */
 ig_status ig_set_compression(ig_ctx* ctx, int on);
 ig_status ig_get_compressed(ig_ctx* ctx, long long* n_compressed);
 /* Pixel commits so far: atomic reductions of one multi-polarised pixel into the grid (the

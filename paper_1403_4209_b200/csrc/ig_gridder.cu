@@ -142,9 +142,8 @@ __device__ __forceinline__ void commit(float* __restrict__ grid, unsigned long l
 // Lanes whose q lies outside the footprint run the same instructions on tap (0,0) with the sentinel
 // pixel -1, which never commits.
 template <int NPOL, int R, bool COUNT>
-__device__ __forceinline__ unsigned grid_run(const char* __restrict__ rp, int n_rec, int S, int q0, bool compress,
-                                             unsigned& n_merged, float* __restrict__ grid,
-                                             const float2* __restrict__ bank, int N) {
+__device__ __forceinline__ unsigned grid_run(const char* __restrict__ rp, int n_rec, int S, int q0,
+                                             float* __restrict__ grid, const float2* __restrict__ bank, int N) {
     constexpr int STRIDE = NPOL == 4 ? 48 : 32;
     const unsigned long long plane_bytes = (unsigned long long)N * N * 16;   // 4 pol: two planes of pol pairs
     f32x2 acc[R][NPOL];
@@ -168,56 +167,18 @@ __device__ __forceinline__ unsigned grid_run(const char* __restrict__ rp, int n_
 #pragma unroll
     for (int k = 0; k < R; ++k) krel[k] = 0;
     uint32_t last_x = 0xffffffffu, last_z = 0xffffffffu;
-    auto load_vis = [](const char* p, float (&v)[2 * NPOL]) {
-        const float4 a = *reinterpret_cast<const float4*>(p + 16);
-        v[0] = a.x; v[1] = a.y;
-        if constexpr (NPOL >= 2) { v[2] = a.z; v[3] = a.w; }
-        if constexpr (NPOL == 4) {
-            const float4 b = *reinterpret_cast<const float4*>(p + 32);
-            v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
-        }
-    };
-    uint4 h = *reinterpret_cast<const uint4*>(rp);
-    int r = 0;
-    const int q_first = q0 - (q0 & 31);                 // first point of this pass (q0 = q_first + lane)
-    const int j_lo = q_first / S;
-    const int n_rows = (min(S * S, q_first + 32 * R) - 1) / S - j_lo + 1;
-    const int lane128 = (q0 & 31) * 128;
 #pragma unroll 1
-    while (r < n_rec) {
+    for (int r = 0; r < n_rec; ++r, rp += STRIDE) {
+        const uint4 h = *reinterpret_cast<const uint4*>(rp);
+        if (h.z & IG_HDR_MERGED) continue;   // compression: ingest summed this record into its predecessor
         float v[2 * NPOL];
-        load_vis(rp + r * STRIDE, v);
-        // Compression (eq 4.9 :1407-1414, eq 4.16): records that follow with the same
-        // cell AND the same kernel matrix (plane and sub-cell offsets) are summed first and gridded once.
-        int rn = r + 1;
-        uint4 hn = h;
-        for (;;) {
-            if (rn >= n_rec) break;
-            hn = *reinterpret_cast<const uint4*>(rp + rn * STRIDE);
-            if (!compress || hn.x != h.x || hn.y != h.y || ((hn.z ^ h.z) & 0x00ffffffu)) break;
-            float w[2 * NPOL];
-            load_vis(rp + rn * STRIDE, w);
-#pragma unroll
-            for (int e = 0; e < 2 * NPOL; ++e) v[e] += w[e];
-            ++rn;
-        }
-        if constexpr (COUNT) n_merged += (q0 < 32) ? (unsigned)(rn - r - 1) : 0u;   // pass 0 only; same on every lane
-        // Prefetch into L1 the part of the NEXT record's kernel matrix that this pass will read: the tap rows
-        // (j + d) mod S of the pass's point rows, one or two contiguous byte ranges, one 128-byte line per lane.
-        // The loads of the next iteration then hit L1 instead of waiting on L2 / HBM (ncu: long-scoreboard
-        // stalls on the first FFMA2 after the LDGs were the top stall, 30 % of samples on config 5).
-        if (rn < n_rec) {
-            int row0 = j_lo + (int)((hn.z >> 8) & 0xffu);
-            row0 = row0 >= S ? row0 - S : row0;
-            const char* mat = reinterpret_cast<const char*>(bank64 + hn.y);
-            const int end1 = min(row0 + n_rows, S);
-            const char* a0 = mat + row0 * S * 8;
-            const char* p0 = reinterpret_cast<const char*>(reinterpret_cast<uintptr_t>(a0) & ~(uintptr_t)127) + lane128;
-            if (p0 < mat + end1 * S * 8) asm volatile("prefetch.global.L1 [%0];" ::"l"(p0));
-            const int wrap = row0 + n_rows - S;            // rows that wrapped to the top of the matrix
-            if (wrap > 0) {
-                const char* p1 = reinterpret_cast<const char*>(reinterpret_cast<uintptr_t>(mat) & ~(uintptr_t)127) + lane128;
-                if (p1 < mat + wrap * S * 8) asm volatile("prefetch.global.L1 [%0];" ::"l"(p1));
+        {
+            const float4 a = *reinterpret_cast<const float4*>(rp + 16);
+            v[0] = a.x; v[1] = a.y;
+            if constexpr (NPOL >= 2) { v[2] = a.z; v[3] = a.w; }
+            if constexpr (NPOL == 4) {
+                const float4 b = *reinterpret_cast<const float4*>(rp + 32);
+                v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
             }
         }
         f32x2 kv[R];
@@ -249,8 +210,6 @@ __device__ __forceinline__ unsigned grid_run(const char* __restrict__ rp, int n_
 #pragma unroll
             for (int q = 0; q < NPOL; ++q) cmac(acc[k][q], v[2 * q], v[2 * q + 1], kv[k]);
         }
-        h = hn;
-        r = rn;
     }
 #pragma unroll
     for (int k = 0; k < R; ++k)
@@ -262,7 +221,7 @@ template <int NPOL, bool COUNT>
 __global__ void __launch_bounds__(IG_GRID_WARPS * 32, IG_GRID_CTAS_PER_SM)
 k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_smax, unsigned nrb, unsigned nchan,
           float* __restrict__ grid, const float2* __restrict__ bank, int N, unsigned* __restrict__ ticket,
-          unsigned long long* __restrict__ commits, unsigned long long* __restrict__ merged, bool compress) {
+          unsigned long long* __restrict__ commits) {
     constexpr int STRIDE = NPOL == 4 ? 48 : 32;
     constexpr int STAGE_BYTES = IG_STAGE * STRIDE;
     __shared__ __align__(128) char sm_rec[IG_GRID_WARPS][IG_CH * STRIDE];
@@ -278,7 +237,7 @@ k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_s
     }
     __syncwarp();
     uint32_t phase = 0;
-    unsigned n_commit = 0, n_merged = 0;
+    unsigned n_commit = 0;
     const unsigned n_chunks = nrb * nchan;
 
     for (;;) {
@@ -334,7 +293,7 @@ k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_s
                 for (int pass = 0; pass < n_pass; ++pass) {
                     const int q0 = pass * 32 * R + lane;
                     switch (R) {
-#define IG_CASE(r) case r: n_commit += grid_run<NPOL, r, COUNT>(rp, r1 - r0, S, q0, compress, n_merged, grid, bank, N); break;
+#define IG_CASE(r) case r: n_commit += grid_run<NPOL, r, COUNT>(rp, r1 - r0, S, q0, grid, bank, N); break;
                         IG_CASE(1) IG_CASE(2)
 #if IG_RMAX >= 3
                         IG_CASE(3)
@@ -363,7 +322,6 @@ k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_s
     if constexpr (COUNT) {
         n_commit = __reduce_add_sync(0xffffffffu, n_commit);
         if (lane == 0 && n_commit) atomicAdd(commits, (unsigned long long)n_commit);
-        if (lane == 0 && n_merged) atomicAdd(merged, (unsigned long long)n_merged);   // counted once per pass 0 only
     }
 }
 
@@ -379,7 +337,7 @@ int ig_launch_gridder(ig_ctx* c, const char* records, const uint32_t* chunk_smax
     long long want = (n_chunks + IG_GRID_WARPS - 1) / IG_GRID_WARPS;
     unsigned ctas = (unsigned)(want < (long long)sms * per_sm ? want : (long long)sms * per_sm);
     dim3 g(ctas), b(IG_GRID_WARPS * 32);
-#define IG_LAUNCH(P, C) k_gridder<P, C><<<g, b, 0, c->stream>>>(records, chunk_smax, (unsigned)nrb, (unsigned)nchan, c->grid, c->d_bank, c->prm.N, &c->d_acc->ticket, &c->d_acc->commits, &c->d_acc->merged, c->compress)
+#define IG_LAUNCH(P, C) k_gridder<P, C><<<g, b, 0, c->stream>>>(records, chunk_smax, (unsigned)nrb, (unsigned)nchan, c->grid, c->d_bank, c->prm.N, &c->d_acc->ticket, &c->d_acc->commits)
     if (c->count_commits) {
         switch (c->prm.npol) { case 1: IG_LAUNCH(1, true); break; case 2: IG_LAUNCH(2, true); break; default: IG_LAUNCH(4, true); break; }
     } else {

@@ -62,7 +62,7 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
         const double* __restrict__ uvw, const uint32_t* __restrict__ perm, long long nrow,
         const double* __restrict__ freqs, int nchan, const float* __restrict__ vis,
         const float* __restrict__ wt, char* __restrict__ records, uint32_t* __restrict__ chunk_smax,
-        IgAccum* __restrict__ acc) {
+        IgAccum* __restrict__ acc, bool compress) {
     constexpr int STRIDE = NPOL == 4 ? 48 : 32;
     const long long rb = blockIdx.x;
     const int t = threadIdx.x, lane = t & 31;
@@ -80,7 +80,7 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
     double nsum[NPOL];
 #pragma unroll
     for (int q = 0; q < NPOL; ++q) nsum[q] = 0.0;
-    unsigned long long n_grid = 0, n_drop = 0, n_upd = 0;
+    unsigned long long n_grid = 0, n_drop = 0, n_upd = 0, n_merged = 0;
 
     for (int c = 0; c < nchan; ++c) {
         const long long chunk = rb * nchan + c;
@@ -131,6 +131,34 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
                 n_drop += 1;
             }
         }
+        // Compression (eq 4.9 :1407-1414, eq 4.16): records that follow one another with
+        // the same cell and the same kernel matrix (plane, sub-cell offsets) are summed into the first of the
+        // group; the others stay in place, flagged, and the gridder skips them. Groups are found among the 32
+        // consecutive rows of a warp (segmented suffix sum by shuffles; warps without a pair skip it).
+        if (compress) {
+            const uint32_t px = __shfl_up_sync(0xffffffffu, hdr.x, 1), py = __shfl_up_sync(0xffffffffu, hdr.y, 1);
+            const uint32_t pz = __shfl_up_sync(0xffffffffu, hdr.z, 1);
+            const bool follows = lane > 0 && S > 0 && px == hdr.x && py == hdr.y && pz == hdr.z;
+            const uint32_t heads = __ballot_sync(0xffffffffu, !follows);
+            if (heads != 0xffffffffu) {
+                const uint32_t after = lane == 31 ? 0u : (heads & (0xffffffffu << (lane + 1)));
+                const int end = after ? __ffs(after) - 2 : 31;     // last lane of this lane's group
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+#pragma unroll
+                    for (int q = 0; q < 2 * NPOL; ++q) {
+                        const float t = __shfl_down_sync(0xffffffffu, v[q], o);
+                        if (lane + o <= end) v[q] += t;
+                    }
+                }
+                if (follows) {
+                    hdr.z |= IG_HDR_MERGED;
+                    n_merged += 1;
+#pragma unroll
+                    for (int q = 0; q < 2 * NPOL; ++q) v[q] = 0.f;
+                }
+            }
+        }
         *reinterpret_cast<uint4*>(rec) = hdr;
         if constexpr (NPOL == 4) {
             *reinterpret_cast<float4*>(rec + 16) = make_float4(v[0], v[1], v[2], v[3]);
@@ -145,7 +173,7 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
     }
 
     // block reduction of the normaliser and the counters
-    __shared__ double sh[IG_CH / 32][NPOL + 3];
+    __shared__ double sh[IG_CH / 32][NPOL + 4];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
 #pragma unroll
@@ -153,20 +181,23 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
         n_grid += __shfl_xor_sync(0xffffffffu, n_grid, o);
         n_drop += __shfl_xor_sync(0xffffffffu, n_drop, o);
         n_upd += __shfl_xor_sync(0xffffffffu, n_upd, o);
+        n_merged += __shfl_xor_sync(0xffffffffu, n_merged, o);
     }
     if (lane == 0) {
 #pragma unroll
         for (int q = 0; q < NPOL; ++q) sh[t >> 5][q] = nsum[q];
         sh[t >> 5][NPOL] = (double)n_grid; sh[t >> 5][NPOL + 1] = (double)n_drop; sh[t >> 5][NPOL + 2] = (double)n_upd;
+        sh[t >> 5][NPOL + 3] = (double)n_merged;
     }
     __syncthreads();
-    if (t < NPOL + 3) {
+    if (t < NPOL + 4) {
         double s = 0;
         for (int w = 0; w < IG_CH / 32; ++w) s += sh[w][t];   // counts < 2^53: exact in fp64
         if (t < NPOL) atomicAdd(&acc->norm[t], s);
         else if (t == NPOL) atomicAdd(&acc->gridded, (unsigned long long)s);
         else if (t == NPOL + 1) atomicAdd(&acc->dropped, (unsigned long long)s);
-        else atomicAdd(&acc->updates, (unsigned long long)s);
+        else if (t == NPOL + 2) atomicAdd(&acc->updates, (unsigned long long)s);
+        else if (s > 0) atomicAdd(&acc->merged, (unsigned long long)s);
     }
 }
 
@@ -192,9 +223,9 @@ int ig_launch_index(ig_ctx* c, const double* uvw, const uint32_t* perm, long lon
     IG_CUDA_OK(c, cudaMemsetAsync(chunk_smax, 0, (size_t)nrb * nchan * 4, c->stream));
     dim3 g((unsigned)nrb), b(IG_CH);
     switch (c->prm.npol) {
-        case 1: k_index<1><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc); break;
-        case 2: k_index<2><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc); break;
-        default: k_index<4><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc); break;
+        case 1: k_index<1><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc, c->compress); break;
+        case 2: k_index<2><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc, c->compress); break;
+        default: k_index<4><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc, c->compress); break;
     }
     IG_CUDA_OK(c, cudaGetLastError());
     return 1;

@@ -18,6 +18,7 @@
 #define IG_GRID_CTAS_PER_SM 4
 #endif
 // IG_GRID_CTAS_PER_SM: launch bound and persistent grid size
+#define IG_HDR_MERGED (1u << 25)   // record header word z: visibility already summed into the run's head record
 #define IG_GRID_WARPS 4      // warps per gridder CTA
 
 // Device-side tail of the bank buffer: small tables and accumulators.
@@ -73,6 +74,7 @@ void ig_taper_eval(const double* eta, int n, double* psi);
 int ig_launch_sort_rows(ig_ctx* c, const double* uvw, const int* baseline_id, long long nrow, double ref_freq_hz,
                         uint32_t* perm_out, char* scratch, size_t scratch_bytes);
 size_t ig_sort_scratch_bytes(long long nrow);
+// (compression is applied in k_index when c->compress is set)
 int ig_launch_index(ig_ctx* c, const double* uvw, const uint32_t* perm, long long nrow,
                     const double* d_freqs, int nchan, const float* vis, const float* wt,
                     char* records, uint32_t* chunk_smax);
