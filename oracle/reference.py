@@ -121,6 +121,21 @@ def oversampled_kernel(p, n_wplanes, w_max, du, beta, n, q_lo, q_hi):
     return (E @ f @ E.T) / A                                # [qv][qu]
 
 
+def kernel_samples(p, n_wplanes, w_max, du, beta, n, qv, qu):
+    """C_p at the listed oversampled sample pairs (qv[k], qu[k]) only: the same direct DFT as
+    oversampled_kernel, evaluated pair by pair (used to check single grid pixels of full-size runs)."""
+    f, A = image_plane_function(p, n_wplanes, w_max, du, n)
+    a = np.arange(-n // 2, n // 2, dtype=np.float64)
+    qv = np.asarray(qv, dtype=np.float64)
+    qu = np.asarray(qu, dtype=np.float64)
+    out = np.empty(qv.size, dtype=np.complex128)
+    for s0 in range(0, qv.size, 256):               # bounded temporaries
+        Ev = np.exp(-2j * np.pi * np.outer(qv[s0:s0 + 256], a) / (beta * n))   # [k][b]
+        Eu = np.exp(-2j * np.pi * np.outer(qu[s0:s0 + 256], a) / (beta * n))   # [k][a]
+        out[s0:s0 + 256] = np.einsum("kb,kb->k", Ev @ f, Eu) / A
+    return out
+
+
 def build_bank(supports, w_max, du, beta, max_support):
     """Returns (bank complex128 flat, bank_off int64[P]).
     K[p][ov][ou][ty][tx] = C_p[ty*beta - off_v][tx*beta - off_u], ty,tx in [-h,h],

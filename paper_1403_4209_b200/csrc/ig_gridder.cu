@@ -203,7 +203,11 @@ __device__ __forceinline__ unsigned grid_run(const char* __restrict__ rp, int n_
                 kv[k] = __ldg(bank64 + (uint32_t)(krel[k] + h.y));            // 32-bit element index
             }
 #pragma unroll
-            for (int k = 0; k < R; ++k) commit_step<NPOL, COUNT>(acc[k], prev[k], pix[k], grid, plane_bytes, n_commit);
+            for (int k = 0; k < R; ++k) {
+                // warp-uniform skip: in about half of the (record, slot) pairs no lane's pixel has changed
+                if (__any_sync(0xffffffffu, pix[k] != prev[k]))
+                    commit_step<NPOL, COUNT>(acc[k], prev[k], pix[k], grid, plane_bytes, n_commit);
+            }
         }
 #pragma unroll
         for (int k = 0; k < R; ++k) {

@@ -284,3 +284,61 @@ def test_compression_same_grid_and_counts(orc, torch_cuda):
     assert merged[False] == 0
     # two of every three records are merged, except where a 128-row work item or a tile edge cuts a triple
     assert 0.6 * nrec <= merged[True] <= (2 * nrec) // 3
+
+
+def _sampled_pixel_check(orc, torch_cuda, cfg_index, n_pixels, seed):
+    """Full-size run of BASELINE.json configs[cfg_index] through the entry point bench.py times; the oracle
+    computes `n_pixels` touched grid pixels one by one from its own indices and its own kernel samples
+    (sum over every record whose footprint covers the pixel, eq 4.4), all polarisations."""
+    cfg = synth.CONFIGS[cfg_index]
+    wl = synth.make_workload(cfg)
+    sup, beta, N, P = wl["supports"], cfg.oversampling, cfg.grid_n, cfg.n_wplanes
+    g = make_gridder(wl)
+    g.build_wkernels(wl["w_max"])
+    uvw, bl, vis, wt = to_dev(torch_cuda, wl)
+    g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+    torch_cuda.cuda.synchronize()
+    del uvw, bl, vis, wt
+    idx = orc.index_records(wl["uvw_m"], wl["freqs_hz"], N, wl["cell_rad"], beta, P, wl["w_max"], sup)
+    X, Y, pl = idx["X"].ravel(), idx["Y"].ravel(), idx["plane"].ravel()
+    ou, ov, fl = idx["off_u"].ravel(), idx["off_v"].ravel(), idx["flags"].ravel()
+    half = ((sup.astype(np.int64) - 1) // 2)[pl].astype(np.int32)
+    visf = wl["vis"].reshape(-1, cfg.n_pol)
+    wtf = wl["weights"].reshape(-1, cfg.n_pol)
+    rng = np.random.default_rng(seed)
+    n_in = orc.inner_samples(int(sup.max()))
+    # pixels: centre cells of random records (touched by construction), a mix of core and long baselines
+    picks = rng.integers(0, X.size, n_pixels)
+    worst = 0.0
+    got_grid = g.grid.view(2, N, N, 2, 2) if cfg.n_pol == 4 else None
+    for k in picks:
+        xp, yp = int(X[k]), int(Y[k])
+        m = (np.abs(X - xp) <= half) & (np.abs(Y - yp) <= half) & ((fl & 2) != 0)
+        r = np.nonzero(m)[0]
+        a = wtf[r].astype(np.float64) * np.where((fl[r] & 1)[:, None] != 0, np.conj(visf[r]), visf[r]).astype(np.complex128)
+        qv = (yp - Y[r]).astype(np.int64) * beta - ov[r]
+        qu = (xp - X[r]).astype(np.int64) * beta - ou[r]
+        want = np.zeros(cfg.n_pol, dtype=np.complex128)
+        for p in np.unique(pl[r]):
+            s = pl[r] == p
+            c = orc.kernel_samples(int(p), P, wl["w_max"], wl["du"], beta, n_in, qv[s], qu[s])
+            want += (a[s] * c[:, None]).sum(axis=0)
+        if cfg.n_pol == 4:
+            gp = got_grid[:, yp, xp].cpu().numpy().astype(np.float64)          # [pair][k][re,im]
+            got = (gp[..., 0] + 1j * gp[..., 1]).reshape(4)
+        else:
+            gp = g.grid[yp, xp].cpu().numpy().astype(np.float64)
+            got = gp[..., 0] + 1j * gp[..., 1]
+        err = np.abs(got - want).max() / max(np.abs(want).max(), 1e-30)
+        worst = max(worst, err)
+        assert err <= 2e-5, (xp, yp, r.size, err)      # fp32 sums of up to ~1e4 terms per pixel against fp64
+    gridded, dropped, updates = g.stats()
+    on = (fl & 2) != 0
+    assert gridded == int(on.sum()) and dropped == int((~on).sum())
+    assert updates == int((sup.astype(np.int64)[pl[on]] ** 2).sum()) * cfg.n_pol
+    return worst
+
+
+def test_full_size_config5_sampled_pixels(orc, torch_cuda):
+    """The configuration bench.py times by default (267.9 M records, 16384^2 x 4 pol, 512 planes)."""
+    _sampled_pixel_check(orc, torch_cuda, 4, n_pixels=4, seed=55)

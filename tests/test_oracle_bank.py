@@ -112,3 +112,14 @@ def test_bank_layout_and_selection(orc):
                         want = C[ty * beta - offv + (h + 1) * beta, tx * beta - offu + (h + 1) * beta]
                         assert K[offv + 1, offu + 1, ty + h, tx + h] == want
     assert bank[off[0] + (1 * beta + 1) * 25 + 2 * 5 + 2] == pytest.approx(1.0, abs=1e-13)  # C_0(0,0) at off=0, centre tap
+
+
+def test_kernel_samples_agree_with_the_plane(orc):
+    """kernel_samples (pair-by-pair DFT) against oversampled_kernel (whole plane) on random sample pairs."""
+    rng = np.random.default_rng(11)
+    P, w_max, du, beta, n = 6, 900.0, 25.0, 4, 32
+    for p in (0, 3, 5):
+        C = orc.oversampled_kernel(p, P, w_max, du, beta, n, -20, 20)
+        qv, qu = rng.integers(-20, 21, 50), rng.integers(-20, 21, 50)
+        got = orc.kernel_samples(p, P, w_max, du, beta, n, qv, qu)
+        assert np.abs(got - C[qv + 20, qu + 20]).max() < 1e-13
