@@ -79,14 +79,14 @@ __device__ __forceinline__ void commit_step(f32x2 (&a)[NPOL], int& prev, int pix
     if constexpr (COUNT) n_commit += (pix != prev && prev >= 0) ? 1u : 0u;
     if constexpr (NPOL == 4) {
         asm volatile(
-            "{\n\t.reg .pred p, q;\n\t.reg .u64 ad;\n\t.reg .f32 f<8>;\n\t"
+            "{\n\t.reg .pred p, q;\n\t.reg .u64 ad, ae;\n\t.reg .f32 f<8>;\n\t"
             "setp.ne.s32 p, %5, %4;\n\t"
             "setp.ge.and.s32 q, %4, 0, p;\n\t"
             "mov.b64 {f0,f1}, %0;\n\tmov.b64 {f2,f3}, %1;\n\tmov.b64 {f4,f5}, %2;\n\tmov.b64 {f6,f7}, %3;\n\t"
-            "@q mad.wide.s32 ad, %4, 16, %6;\n\t"
+            "mad.wide.s32 ad, %4, 16, %6;\n\t"
+            "add.u64 ae, ad, %7;\n\t"
             "@q red.global.add.v4.f32 [ad], {f0,f1,f2,f3};\n\t"
-            "@q add.u64 ad, ad, %7;\n\t"
-            "@q red.global.add.v4.f32 [ad], {f4,f5,f6,f7};\n\t"
+            "@q red.global.add.v4.f32 [ae], {f4,f5,f6,f7};\n\t"
             "@p mov.b64 %0, 0;\n\t@p mov.b64 %1, 0;\n\t@p mov.b64 %2, 0;\n\t@p mov.b64 %3, 0;\n\t"
             "@p mov.s32 %4, %5;\n\t}"
             : "+l"(a[0]), "+l"(a[1]), "+l"(a[2]), "+l"(a[3]), "+r"(prev)

@@ -15,7 +15,7 @@
 // IG_RMAX: grid points per lane, at most (tunable with -DIG_RMAX for experiments)
 #define IG_TIMING_RING 64    // ig_grid calls whose event triples are kept
 #ifndef IG_GRID_CTAS_PER_SM
-#define IG_GRID_CTAS_PER_SM 4
+#define IG_GRID_CTAS_PER_SM 5
 #endif
 // IG_GRID_CTAS_PER_SM: launch bound and persistent grid size
 #define IG_HDR_MERGED (1u << 25)   // record header word z: visibility already summed into the run's head record
