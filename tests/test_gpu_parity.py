@@ -38,6 +38,8 @@ CASES = {
     "cfg4s": small(synth.CONFIGS[3], grid_n=2048, n_station=8, n_time=130, n_chan=6, n_wplanes=20),
     "cfg5s": small(synth.CONFIGS[4], grid_n=2048, n_station=9, n_time=128, n_chan=5, n_wplanes=16, s_max=129),
     "pol2": small(synth.CONFIGS[1], n_pol=2, n_station=9, n_time=77, n_chan=3, n_wplanes=8),
+    # grid side that is not a power of two (the thesis images 4500^2, :1988), odd row count, 1 polarisation
+    "n300": small(synth.CONFIGS[1], grid_n=300, n_pol=1, n_station=7, n_time=61, n_chan=2, n_wplanes=5, s_max=21),
 }
 
 
@@ -203,7 +205,7 @@ def test_host_entry_point_and_empty_input(runs, torch_cuda):
     check_grid(g.grid_complex(), ref["grid"])
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg2s"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg2s", "n300"])
 def test_finalize_matches_oracle(name, runs, orc, torch_cuda):
     wl, ref = runs(name)
     cfg = wl["cfg"]
