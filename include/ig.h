@@ -115,6 +115,10 @@ ig_status ig_grid(ig_ctx* ctx, const double* uvw_m, const int* baseline_id, long
 /* Same, with HOST inputs: copies them to staging areas inside work_dev (which must be
  * ig_workspace_bytes() + ig_host_staging_bytes() large) and grids. The end-to-end leg. */
 size_t ig_host_staging_bytes(const ig_ctx* ctx, long long nrow, int nchan);
+/* ig_grid_host cuts the rows into n slices (default 8; 1 = no slicing; batches under 65 536 rows are never
+ * sliced) and copies slice k+1 on a second stream while slice k is gridded. The copies overlap the kernels only
+ * when the host buffers are pinned. More slices shorten the tracks inside a slice (more commits). */
+ig_status ig_set_host_slices(ig_ctx* ctx, int n);
 ig_status ig_grid_host(ig_ctx* ctx, const double* uvw_m, const int* baseline_id, long long nrow,
                        const double* freqs_hz, int nchan, const float* vis, const float* weights);
 

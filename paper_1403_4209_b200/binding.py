@@ -32,6 +32,7 @@ SIGNATURES = {
     "ig_debug_get_wkernels": (_i, [_vp, _vp, _sz]),
     "ig_grid": (_i, [_vp, _vp, _vp, _ll, _vp, _i, _vp, _vp]),
     "ig_host_staging_bytes": (_sz, [_vp, _ll, _i]),
+    "ig_set_host_slices": (_i, [_vp, _i]),
     "ig_grid_host": (_i, [_vp, _vp, _vp, _ll, _vp, _i, _vp, _vp]),
     "ig_finalize": (_i, [_vp, _vp, _vp]),
     "ig_get_stats": (_i, [_vp, C.POINTER(_ll), C.POINTER(_ll), C.POINTER(_ll)]),
@@ -194,6 +195,9 @@ class Gridder:
         g, d, u = _ll(), _ll(), _ll()
         self._check(self.lib.ig_get_stats(self.ctx, C.byref(g), C.byref(d), C.byref(u)), "ig_get_stats")
         return g.value, d.value, u.value
+
+    def set_host_slices(self, n: int):
+        self._check(self.lib.ig_set_host_slices(self.ctx, int(n)), "ig_set_host_slices")
 
     def set_compression(self, on: bool):
         self._check(self.lib.ig_set_compression(self.ctx, int(bool(on))), "ig_set_compression")

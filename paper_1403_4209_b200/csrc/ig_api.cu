@@ -88,6 +88,9 @@ ig_status ig_create(ig_ctx** out, int grid_n, double cell_rad, int n_wplanes, in
 void ig_destroy(ig_ctx* c) {
     if (!c) return;
     for (auto& t : c->ev) for (auto& e : t) if (e) cudaEventDestroy(e);
+    for (auto& e : c->ev_copied) if (e) cudaEventDestroy(e);
+    for (auto& e : c->ev_free) if (e) cudaEventDestroy(e);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     delete c;
 }
 
@@ -106,8 +109,9 @@ size_t ig_bank_bytes(const ig_ctx* c, const int* table) {
 size_t ig_finalize_workspace_bytes(const ig_ctx* c) { return c ? ig_finalize_scratch_bytes(c) : 0; }
 size_t ig_host_staging_bytes(const ig_ctx* c, long long nrow, int nchan) {
     if (!c || nrow < 0 || nchan < 1) return 0;
+    // room for an unsliced copy of everything: an upper bound for any slice count (two slice buffers need less)
     size_t rec = (size_t)nrow * nchan * c->prm.npol;
-    return ig_align((size_t)nrow * 24) + ig_align((size_t)nrow * 4) + ig_align(rec * 8) + ig_align(rec * 4);
+    return ig_align((size_t)nrow * 24) + ig_align((size_t)nrow * 4) + ig_align(rec * 8) + ig_align(rec * 4) + 4096;
 }
 
 ig_status ig_bind(ig_ctx* c, void* grid_dev, size_t grid_bytes, void* work_dev, size_t work_bytes, void* bank_dev,
@@ -223,6 +227,26 @@ ig_status ig_grid(ig_ctx* c, const double* uvw, const int* baseline_id, long lon
     return IG_OK;
 }
 
+// Host entry point: the rows are cut into `host_slices` slices; slice k+1 is copied (second stream, double
+// buffered staging inside work_dev) while slice k is ordered, indexed and gridded. ig_grid is additive, so the
+// slices need no merge step. The copies overlap the kernels only if the caller's buffers are pinned.
+static long long host_slice_rows(const ig_ctx* c, long long nrow) {
+    int k = c->host_slices;
+    if (nrow < (1 << 16)) k = 1;
+    long long r = (nrow + k - 1) / k;
+    return (r + IG_CH - 1) / IG_CH * IG_CH;          // whole row blocks
+}
+static size_t host_stage_bytes(const ig_ctx* c, long long rows, int nchan) {
+    size_t rec = (size_t)rows * nchan * c->prm.npol;
+    return ig_align((size_t)rows * 24) + ig_align((size_t)rows * 4) + ig_align(rec * 8) + ig_align(rec * 4);
+}
+
+ig_status ig_set_host_slices(ig_ctx* c, int n) {
+    if (!c || n < 1 || n > 1024) return IG_EINVAL;
+    c->host_slices = n;
+    return IG_OK;
+}
+
 ig_status ig_grid_host(ig_ctx* c, const double* uvw, const int* baseline_id, long long nrow, const double* freqs,
                        int nchan, const float* vis, const float* wt) {
     if (!c) return IG_EINVAL;
@@ -230,20 +254,46 @@ ig_status ig_grid_host(ig_ctx* c, const double* uvw, const int* baseline_id, lon
     if (nrow < 0 || nchan < 1) return fail(c, IG_EINVAL, "bad nrow/nchan");
     if (nrow == 0) return IG_OK;
     if (!uvw || !baseline_id || !vis || !wt) return fail(c, IG_EINVAL, "null input");
-    size_t base = ig_align(grid_layout(c, nrow, nchan).total);
-    if (base + ig_host_staging_bytes(c, nrow, nchan) > c->work_bytes) return fail(c, IG_ENOMEM, "work buffer smaller than ig_workspace_bytes() + ig_host_staging_bytes()");
-    size_t rec = (size_t)nrow * nchan * c->prm.npol;
-    char* p = c->work + base;
-    double* d_uvw = (double*)p; p += ig_align((size_t)nrow * 24);
-    int* d_bl = (int*)p; p += ig_align((size_t)nrow * 4);
-    float* d_vis = (float*)p; p += ig_align(rec * 8);
-    float* d_wt = (float*)p;
-    cudaError_t e = cudaMemcpyAsync(d_uvw, uvw, (size_t)nrow * 24, cudaMemcpyHostToDevice, c->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d_bl, baseline_id, (size_t)nrow * 4, cudaMemcpyHostToDevice, c->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d_vis, vis, rec * 8, cudaMemcpyHostToDevice, c->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d_wt, wt, rec * 4, cudaMemcpyHostToDevice, c->stream);
+    const long long srows = host_slice_rows(c, nrow);
+    const size_t base = ig_align(grid_layout(c, srows, nchan).total);
+    const size_t stage = host_stage_bytes(c, srows, nchan);
+    const int nbuf = srows < nrow ? 2 : 1;
+    if (base + nbuf * stage > c->work_bytes) return fail(c, IG_ENOMEM, "work buffer smaller than ig_workspace_bytes() + ig_host_staging_bytes()");
+    if (!c->copy_stream) {
+        if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(c, IG_ECUDA, "cannot create the copy stream");
+        for (auto& e : c->ev_copied) cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+        for (auto& e : c->ev_free) cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+    }
+    // the staging area may still be in use by work queued earlier on the bound stream
+    cudaError_t e = cudaEventRecord(c->ev_free[0], c->stream);
+    if (e == cudaSuccess) e = cudaEventRecord(c->ev_free[1], c->stream);
     if (e != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_grid_host: ") + cudaGetErrorString(e));
-    return ig_grid(c, d_uvw, d_bl, nrow, freqs, nchan, d_vis, d_wt);
+    const size_t vrow = (size_t)nchan * c->prm.npol;     // visibilities per row
+    int launches = 0, k = 0;
+    for (long long r0 = 0; r0 < nrow; r0 += srows, ++k) {
+        const long long rows = (nrow - r0 < srows) ? nrow - r0 : srows;
+        const int b = k & 1;
+        char* p = c->work + base + (size_t)b * stage;
+        double* d_uvw = (double*)p; p += ig_align((size_t)srows * 24);
+        int* d_bl = (int*)p; p += ig_align((size_t)srows * 4);
+        float* d_vis = (float*)p; p += ig_align((size_t)srows * vrow * 8);
+        float* d_wt = (float*)p;
+        e = cudaStreamWaitEvent(c->copy_stream, c->ev_free[b], 0);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(d_uvw, uvw + 3 * r0, (size_t)rows * 24, cudaMemcpyHostToDevice, c->copy_stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(d_bl, baseline_id + r0, (size_t)rows * 4, cudaMemcpyHostToDevice, c->copy_stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(d_vis, vis + (size_t)r0 * vrow * 2, (size_t)rows * vrow * 8, cudaMemcpyHostToDevice, c->copy_stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(d_wt, wt + (size_t)r0 * vrow, (size_t)rows * vrow * 4, cudaMemcpyHostToDevice, c->copy_stream);
+        if (e == cudaSuccess) e = cudaEventRecord(c->ev_copied[b], c->copy_stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(c->stream, c->ev_copied[b], 0);
+        if (e != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_grid_host: ") + cudaGetErrorString(e));
+        ig_status st = ig_grid(c, d_uvw, d_bl, rows, freqs, nchan, d_vis, d_wt);
+        if (st != IG_OK) return st;
+        launches += c->launches;
+        e = cudaEventRecord(c->ev_free[b], c->stream);
+        if (e != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_grid_host: ") + cudaGetErrorString(e));
+    }
+    c->launches = launches;
+    return IG_OK;
 }
 
 ig_status ig_finalize(ig_ctx* c, float* image_dev, double* norm_host) {

@@ -48,6 +48,9 @@ struct ig_ctx {
     char* bank_buf = nullptr; size_t bank_bytes = 0;
     cudaStream_t stream = nullptr;
     bool bound = false, have_bank = false;
+    int host_slices = 8;                      // ig_set_host_slices
+    cudaStream_t copy_stream = nullptr;       // ig_grid_host: H2D copies of the next slice
+    cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
     bool compress = true;                     // ig_set_compression
     bool count_commits = false;               // ig_set_commit_counting
     // bank description (host copies)

@@ -253,6 +253,12 @@ def test_full_size_config2_whole_grid(orc, torch_cuda):
     g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
     check_grid(g.grid_complex(), ref["grid"])
     assert g.touched_pixels() == int((np.abs(ref["grid"]).sum(axis=2) != 0).sum())
+    # host entry point, rows cut into 3 slices copied on the second stream while the previous slice is gridded
+    g.reset()
+    g.set_host_slices(3)
+    g.grid_visibilities_host(wl["uvw_m"], wl["baseline"], wl["freqs_hz"], np.ascontiguousarray(wl["vis"]), wl["weights"])
+    check_grid(g.grid_complex(), ref["grid"])
+    assert g.stats() == tuple(int(x) for x in ref["stats"])
 
 
 def test_compression_same_grid_and_counts(orc, torch_cuda):
