@@ -48,17 +48,19 @@ k_sort_hist(const uint64_t* __restrict__ keys, long long n, int shift, uint32_t*
     uint32_t t = 0;
 #pragma unroll
     for (int w = 0; w < SORT_WARPS; ++w) t += cnt[w][threadIdx.x];
-    hist[(size_t)threadIdx.x * nblk + blockIdx.x] = t;   // bin-major: a flat scan gives global offsets
+    hist[(size_t)threadIdx.x * nblk + blockIdx.x] = t;   // bin-major: rows are scanned per bin, bin totals give the bin starts
 }
 
-// in-place exclusive scan of m uint32 values, one CTA of 1024 threads
-__global__ void __launch_bounds__(1024) k_scan_excl(uint32_t* __restrict__ a, long long m) {
+// in-place exclusive scan of rows of m uint32 values, one CTA (any multiple of 32 threads) per row;
+// the row total goes to totals[row] when totals != nullptr
+__global__ void __launch_bounds__(1024) k_scan_excl(uint32_t* __restrict__ a_all, long long m, uint32_t* __restrict__ totals) {
     __shared__ uint32_t wsum[32];
     __shared__ uint32_t carry_s;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t* a = a_all + (size_t)blockIdx.x * m;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
     if (threadIdx.x == 0) carry_s = 0;
     __syncthreads();
-    for (long long t0 = 0; t0 < m; t0 += 4096) {
+    for (long long t0 = 0; t0 < m; t0 += 4 * blockDim.x) {
         long long i = t0 + (long long)threadIdx.x * 4;
         uint32_t v[4];
 #pragma unroll
@@ -72,13 +74,13 @@ __global__ void __launch_bounds__(1024) k_scan_excl(uint32_t* __restrict__ a, lo
         if (lane == 31) wsum[warp] = inc;
         __syncthreads();
         if (warp == 0) {
-            uint32_t w = wsum[lane], wi = w;
+            uint32_t w = lane < nwarp ? wsum[lane] : 0u, wi = w;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
                 uint32_t y = __shfl_up_sync(0xffffffffu, wi, o);
                 if (lane >= o) wi += y;
             }
-            wsum[lane] = wi - w;   // exclusive over warps
+            wsum[lane] = wi - w;   // exclusive over warps; wsum[nwarp..] hold the tile total
         }
         __syncthreads();
         uint32_t carry = carry_s;
@@ -89,20 +91,21 @@ __global__ void __launch_bounds__(1024) k_scan_excl(uint32_t* __restrict__ a, lo
             ex += v[k];
         }
         __syncthreads();
-        if (threadIdx.x == 1023) carry_s = carry + wsum[31] + inc;
+        if (threadIdx.x == blockDim.x - 1) carry_s = carry + wsum[warp] + inc;
         __syncthreads();
     }
+    if (totals && threadIdx.x == 0) totals[blockIdx.x] = carry_s;
 }
 
 // vals_in == nullptr means the identity permutation (first pass)
 __global__ void __launch_bounds__(SORT_THREADS)
 k_sort_scatter(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ vals_in, long long n, int shift,
-               const uint32_t* __restrict__ hist, int nblk, uint64_t* __restrict__ keys_out,
-               uint32_t* __restrict__ vals_out) {
+               const uint32_t* __restrict__ hist, const uint32_t* __restrict__ binbase, int nblk,
+               uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out) {
     __shared__ uint32_t cnt[SORT_WARPS][256];
     tile_count(keys, n, shift, cnt);
     {   // turn per-warp counts into per-warp start positions in the output
-        uint32_t run = hist[(size_t)threadIdx.x * nblk + blockIdx.x];
+        uint32_t run = binbase[threadIdx.x] + hist[(size_t)threadIdx.x * nblk + blockIdx.x];
 #pragma unroll
         for (int w = 0; w < SORT_WARPS; ++w) {
             uint32_t c = cnt[w][threadIdx.x];
@@ -156,7 +159,7 @@ size_t ig_sort_scratch_bytes(long long nrow) {
     long long nblk = (nrow + SORT_TILE - 1) / SORT_TILE;
     if (nblk < 1) nblk = 1;
     // keysA, keysB (u64), valsB (valsA is the caller's perm_out), hist
-    return 2 * ig_align((size_t)nrow * 8) + ig_align((size_t)nrow * 4) + ig_align((size_t)nblk * 256 * 4);
+    return 2 * ig_align((size_t)nrow * 8) + ig_align((size_t)nrow * 4) + ig_align((size_t)nblk * 256 * 4) + 1024;
 }
 
 int ig_launch_sort_rows(ig_ctx* c, const double* uvw, const int* baseline_id, long long nrow, double ref_freq_hz,
@@ -170,6 +173,7 @@ int ig_launch_sort_rows(ig_ctx* c, const double* uvw, const int* baseline_id, lo
     uint64_t* keysB = (uint64_t*)(scratch + a8);
     uint32_t* valsB = (uint32_t*)(scratch + 2 * a8);
     uint32_t* hist = (uint32_t*)(scratch + 2 * a8 + a4);
+    uint32_t* binbase = hist + (size_t)nblk * 256;        // 256 bin totals, scanned to bin start offsets
     uint32_t* valsA = perm_out;
     // 8 x 8 tiles (tile = N/8 cells, at least 128): measured best on configs 4 and 5 (tiles of 1/16..1/4 of
     // the grid side are within 1 %), no effect on the small grids; finer tiles cut too many tracks and make
@@ -187,9 +191,10 @@ int ig_launch_sort_rows(ig_ctx* c, const double* uvw, const int* baseline_id, lo
         uint64_t* kout = (pass & 1) ? keysA : keysB;
         uint32_t* vout = (pass & 1) ? valsA : valsB;
         k_sort_hist<<<nblk, SORT_THREADS, 0, c->stream>>>(kin, nrow, pass * 8, hist, nblk);
-        k_scan_excl<<<1, 1024, 0, c->stream>>>(hist, (long long)nblk * 256);
-        k_sort_scatter<<<nblk, SORT_THREADS, 0, c->stream>>>(kin, vin, nrow, pass * 8, hist, nblk, kout, vout);
-        launches += 3;
+        k_scan_excl<<<256, 256, 0, c->stream>>>(hist, (long long)nblk, binbase);      // one CTA per bin row
+        k_scan_excl<<<1, 256, 0, c->stream>>>(binbase, 256, nullptr);
+        k_sort_scatter<<<nblk, SORT_THREADS, 0, c->stream>>>(kin, vin, nrow, pass * 8, hist, binbase, nblk, kout, vout);
+        launches += 4;
     }
     IG_CUDA_OK(c, cudaGetLastError());
     return launches;   // result is in valsA == perm_out after the 6th pass
