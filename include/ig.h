@@ -83,10 +83,15 @@ ig_status ig_bind(ig_ctx* ctx, void* grid_dev, size_t grid_bytes, void* work_dev
  *   w_p = w_max (p/(P-1))^2, C_0(0,0) = 1, psi = prolate-spheroidal taper (reading 6),
  *   K[p][ov][ou][ty][tx] = C_p[ty*beta - off_v][tx*beta - off_u], complex64, each S_p x S_p
  *   matrix contiguous (layout C-1 :1100-1108), plus zeta sums (eq 4.3) kept on the device.
- *   support_table  host [n_wplanes], odd, 1..max_support. NULL = IG_EUNSUPPORTED for now
- *                  (auto 1e-3 rule :1114 is "next").
+ *   support_table  host [n_wplanes], odd, 1..max_support. NULL = automatic (:1062,:1114, reading 7): per plane
+ *                  r = largest |q| on either axis through the centre with |C_p| > 1e-3 (C_0 peak = 1) among
+ *                  |q| <= beta*(max_support-1)/2, S_p = 2*ceil(r/beta)+1; bank_dev must then hold
+ *                  ig_bank_bytes(ctx, NULL); the call synchronises; read the result with ig_get_supports.
  * Uses work_dev as scratch. Asynchronous. */
 ig_status ig_build_wkernels(ig_ctx* ctx, double w_max_lambda, const int* support_table);
+
+/* The support table in use (host int[n_wplanes]). */
+ig_status ig_get_supports(ig_ctx* ctx, int* support_table);
 
 /* Test hook: install a bank computed elsewhere (the oracle's), same layout, complex64
  * as float pairs, host memory; zeta sums are recomputed from it. Sets w_max too. */

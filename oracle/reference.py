@@ -136,6 +136,24 @@ def kernel_samples(p, n_wplanes, w_max, du, beta, n, qv, qu):
     return out
 
 
+def auto_supports(n_wplanes, w_max, du, beta, max_support, threshold=1e-3):
+    """Automatic support per plane (reading 7): r = largest |q| on the u-axis row or the
+    v-axis column through the centre with |C_p| > threshold (C_0(0,0) = 1), searched over
+    |q| <= beta*(max_support-1)/2; S = 2*ceil(r/beta)+1."""
+    n = inner_samples(int(max_support))
+    qmax = beta * ((max_support - 1) // 2)
+    q = np.arange(-qmax, qmax + 1)
+    zero = np.zeros_like(q)
+    out = np.empty(n_wplanes, dtype=np.int32)
+    for p in range(n_wplanes):
+        cu = np.abs(kernel_samples(p, n_wplanes, w_max, du, beta, n, zero, q))
+        cv = np.abs(kernel_samples(p, n_wplanes, w_max, du, beta, n, q, zero))
+        over = (cu > threshold) | (cv > threshold)
+        r = int(np.abs(q[over]).max()) if over.any() else 0
+        out[p] = min(max_support, 2 * (-(-r // beta)) + 1)
+    return out
+
+
 def build_bank(supports, w_max, du, beta, max_support):
     """Returns (bank complex128 flat, bank_off int64[P]).
     K[p][ov][ou][ty][tx] = C_p[ty*beta - off_v][tx*beta - off_u], ty,tx in [-h,h],

@@ -28,6 +28,7 @@ SIGNATURES = {
     "ig_finalize_workspace_bytes": (_sz, [_vp]),
     "ig_bind": (_i, [_vp, _vp, _sz, _vp, _sz, _vp, _sz, _vp]),
     "ig_build_wkernels": (_i, [_vp, _d, _vp]),
+    "ig_get_supports": (_i, [_vp, _vp]),
     "ig_debug_set_wkernels": (_i, [_vp, _d, _vp, _vp, _sz]),
     "ig_debug_get_wkernels": (_i, [_vp, _vp, _sz]),
     "ig_grid": (_i, [_vp, _vp, _vp, _ll, _vp, _i, _vp, _vp]),
@@ -127,12 +128,13 @@ class Gridder:
     def allocate(self, supports, work_bytes=0):
         """Allocate grid (zeroed), bank and a work buffer of at least `work_bytes`."""
         t = self.torch
-        supports = np.ascontiguousarray(supports, dtype=np.int32)
-        assert supports.size == self.n_wplanes
-        self.supports = supports
+        if supports is not None:
+            supports = np.ascontiguousarray(supports, dtype=np.int32)
+            assert supports.size == self.n_wplanes
+        self.supports = supports          # None: automatic supports, known after build_wkernels
         with t.cuda.device(self.device):
             self.grid = t.zeros((self.grid_n, self.grid_n, self.n_pol, 2), dtype=t.float32, device=self.device)
-            nb = self.lib.ig_bank_bytes(self.ctx, _np_ptr(supports))
+            nb = self.lib.ig_bank_bytes(self.ctx, _np_ptr(supports) if supports is not None else None)
             self.bank = t.empty(nb, dtype=t.uint8, device=self.device)
             need = max(int(work_bytes), self.lib.ig_workspace_bytes(self.ctx, 0, 1), 1 << 20)
             self.work = t.empty(need, dtype=t.uint8, device=self.device)
@@ -152,7 +154,11 @@ class Gridder:
 
     # -- the calls of include/ig.h ----------------------------------------------------
     def build_wkernels(self, w_max):
-        self._check(self.lib.ig_build_wkernels(self.ctx, float(w_max), _np_ptr(self.supports)), "ig_build_wkernels")
+        tab = _np_ptr(self.supports) if self.supports is not None else None
+        self._check(self.lib.ig_build_wkernels(self.ctx, float(w_max), tab), "ig_build_wkernels")
+        out = np.zeros(self.n_wplanes, dtype=np.int32)
+        self._check(self.lib.ig_get_supports(self.ctx, _np_ptr(out)), "ig_get_supports")
+        self.supports = out
 
     def debug_set_wkernels(self, w_max, bank_c64: np.ndarray):
         b = np.ascontiguousarray(bank_c64, dtype=np.complex64)

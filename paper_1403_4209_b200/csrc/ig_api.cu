@@ -154,14 +154,27 @@ static ig_status set_wmax(ig_ctx* c, double w_max) {
 ig_status ig_build_wkernels(ig_ctx* c, double w_max, const int* table) {
     if (!c) return IG_EINVAL;
     if (!c->bound) return fail(c, IG_ESTATE, "ig_bind first");
-    if (!table) return fail(c, IG_EUNSUPPORTED, "automatic support detection is not implemented; pass a support table");
-    if (!table_ok(c, table)) return fail(c, IG_EINVAL, "supports must be odd and within [1, max_support]");
     ig_status s = set_wmax(c, w_max);
     if (s != IG_OK) return s;
+    std::vector<int> detected;
+    if (!table) {                       // automatic supports: the thesis's 1e-3 rule (:1114), reading 7
+        detected.resize(c->prm.P);
+        if (ig_detect_supports(c, c->work, c->work_bytes, detected.data()) < 0)
+            return c->err.find("too small") != std::string::npos ? IG_ENOMEM : IG_ECUDA;
+        table = detected.data();
+    }
+    if (!table_ok(c, table)) return fail(c, IG_EINVAL, "supports must be odd and within [1, max_support]");
     int r = install_table(c, table);
     if (r < 0) return r == -2 ? IG_ENOMEM : IG_ECUDA;
     if (ig_launch_bank(c, c->work, c->work_bytes) < 0) return c->err.find("too small") != std::string::npos ? IG_ENOMEM : IG_ECUDA;
     c->have_bank = true;
+    return IG_OK;
+}
+
+ig_status ig_get_supports(ig_ctx* c, int* table) {
+    if (!c || !table) return IG_EINVAL;
+    if (!c->have_bank) return fail(c, IG_ESTATE, "no bank");
+    for (int p = 0; p < c->prm.P; ++p) table[p] = c->support[p];
     return IG_OK;
 }
 

@@ -196,6 +196,82 @@ int ig_launch_zeta(ig_ctx* c) {
     return 1;
 }
 
+// ---------------------------------------------------------------------------------------
+// Automatic support ("the pixel nearest to the edge with magnitude > 1e-3", reading 7):
+// r_p = largest |q| (oversampled samples) on either axis through the centre with |C_p| > 1e-3 (C_0 peak = 1),
+// searched over |q| <= beta*(max_support-1)/2; S_p = 2*ceil(r_p/beta) + 1. The axis profiles are 1-D DFTs of
+// the column / row sums of f_p:  C_p[0][q] = sum_a (sum_b f[b][a]) W^(q a) / A.
+__global__ void k_axis_sums(const double2* __restrict__ f, int n, double2* __restrict__ colsum, double2* __restrict__ rowsum) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double cr = 0, ci = 0, rr = 0, ri = 0;
+    for (int k = 0; k < n; ++k) {
+        double2 c = f[(size_t)k * n + i], r = f[(size_t)i * n + k];
+        cr += c.x; ci += c.y; rr += r.x; ri += r.y;
+    }
+    colsum[i] = make_double2(cr, ci);
+    rowsum[i] = make_double2(rr, ri);
+}
+__global__ void k_axis_radius(const double2* __restrict__ colsum, const double2* __restrict__ rowsum,
+                              const double2* __restrict__ W, int n, int M, int qmax, double inv_a, double thr2,
+                              int* __restrict__ radius) {
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t > 2 * qmax) return;
+    const long long q = t - qmax;
+    long long ph = ((q * (long long)(-n / 2)) % M + M) % M;
+    const long long step = ((q % M) + M) % M;
+    double ur = 0, ui = 0, vr = 0, vi = 0;
+    for (int a = 0; a < n; ++a) {
+        const double2 w = W[ph], c = colsum[a], r = rowsum[a];
+        ur += c.x * w.x - c.y * w.y; ui += c.x * w.y + c.y * w.x;
+        vr += r.x * w.x - r.y * w.y; vi += r.x * w.y + r.y * w.x;
+        ph += step; if (ph >= M) ph -= M;
+    }
+    ur *= inv_a; ui *= inv_a; vr *= inv_a; vi *= inv_a;
+    const bool over = (ur * ur + ui * ui > thr2) || (vr * vr + vi * vi > thr2);
+    if (over) atomicMax(radius, (int)(q < 0 ? -q : q));
+}
+
+// Fills table[P] (host) with the detected supports. Synchronises.
+int ig_detect_supports(ig_ctx* c, char* scratch, size_t scratch_bytes, int* table) {
+    if (scratch_bytes < ig_bank_scratch_bytes(c)) { c->err = "work buffer too small for the bank builder"; return -1; }
+    const int n = bank_inner_samples(c->max_support), beta = c->prm.beta, M = n * beta, P = c->prm.P;
+    double* d_psi = (double*)scratch;
+    double2* d_W = (double2*)(scratch + ig_align((size_t)n * 8));
+    double2* d_f = (double2*)((char*)d_W + ig_align((size_t)M * 16));
+    char* g = (char*)d_f + ig_align((size_t)n * n * 16);          // the G area of the builder, free here
+    double2* d_col = (double2*)g;
+    double2* d_row = d_col + n;
+    int* d_rad = (int*)(d_row + n);
+    if ((size_t)n * 32 + (size_t)P * 4 > ig_align((size_t)c->max_support * beta * n * 16)) { c->err = "too many w-planes for the scratch area"; return -1; }
+    std::vector<double> eta(n), psi(n);
+    for (int i = 0; i < n; ++i) eta[i] = 2.0 * (double)(i - n / 2) / (double)n;
+    ig_taper_eval(eta.data(), n, psi.data());
+    double sum = 0;
+    for (int i = 0; i < n; ++i) sum += psi[i];
+    const double inv_a = 1.0 / (sum * sum);
+    IG_CUDA_OK(c, cudaMemcpyAsync(d_psi, psi.data(), (size_t)n * 8, cudaMemcpyHostToDevice, c->stream));
+    IG_CUDA_OK(c, cudaMemsetAsync(d_rad, 0, (size_t)P * 4, c->stream));
+    IG_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    k_bank_twiddle<<<(M + 255) / 256, 256, 0, c->stream>>>(d_W, M);
+    const int qmax = beta * ((c->max_support - 1) / 2);
+    for (int p = 0; p < P; ++p) {
+        const double w = P == 1 ? 0.0 : c->w_max * ((double)p / (P - 1)) * ((double)p / (P - 1));
+        k_bank_f<<<dim3((n + 127) / 128, n), 128, 0, c->stream>>>(d_f, d_psi, n, c->du, w);
+        k_axis_sums<<<(n + 127) / 128, 128, 0, c->stream>>>(d_f, n, d_col, d_row);
+        k_axis_radius<<<(2 * qmax + 1 + 127) / 128, 128, 0, c->stream>>>(d_col, d_row, d_W, n, M, qmax, inv_a, 1e-3 * 1e-3, d_rad + p);
+    }
+    IG_CUDA_OK(c, cudaGetLastError());
+    std::vector<int> rad(P);
+    IG_CUDA_OK(c, cudaMemcpyAsync(rad.data(), d_rad, (size_t)P * 4, cudaMemcpyDeviceToHost, c->stream));
+    IG_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    for (int p = 0; p < P; ++p) {
+        int S = 2 * ((rad[p] + beta - 1) / beta) + 1;
+        table[p] = S > c->max_support ? c->max_support : S;
+    }
+    return 3 * P + 1;
+}
+
 int ig_launch_bank(ig_ctx* c, char* scratch, size_t scratch_bytes) {
     if (scratch_bytes < ig_bank_scratch_bytes(c)) { c->err = "work buffer too small for the bank builder"; return -1; }
     const int n = bank_inner_samples(c->max_support), beta = c->prm.beta, M = n * beta;

@@ -87,6 +87,7 @@ int ig_launch_gridder(ig_ctx* c, const char* records, const uint32_t* chunk_smax
 int ig_launch_bank(ig_ctx* c, char* scratch, size_t scratch_bytes);
 size_t ig_bank_scratch_bytes(const ig_ctx* c);
 int ig_launch_zeta(ig_ctx* c);
+int ig_detect_supports(ig_ctx* c, char* scratch, size_t scratch_bytes, int* table);
 int ig_run_finalize(ig_ctx* c, float* image, double* norm_host);
 size_t ig_finalize_scratch_bytes(const ig_ctx* c);
 

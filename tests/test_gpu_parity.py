@@ -350,3 +350,27 @@ def _sampled_pixel_check(orc, torch_cuda, cfg_index, n_pixels, seed):
 def test_full_size_config5_sampled_pixels(orc, torch_cuda):
     """The configuration bench.py times by default (267.9 M records, 16384^2 x 4 pol, 512 planes)."""
     _sampled_pixel_check(orc, torch_cuda, 4, n_pixels=4, seed=55)
+
+
+def test_automatic_supports_match_oracle_and_grid(orc, torch_cuda):
+    """ig_build_wkernels(NULL table): supports by the 1e-3 rule equal the oracle's (integers, bit-exact), and the
+    whole path with them matches the oracle that uses the oracle's own automatic table."""
+    from paper_1403_4209_b200.binding import Gridder
+    cfg = small(synth.CONFIGS[2], grid_n=512, n_station=8, n_time=90, n_chan=4, n_wplanes=12)
+    wl = synth.make_workload(cfg)
+    max_support = 41
+    want = orc.auto_supports(cfg.n_wplanes, wl["w_max"], wl["du"], cfg.oversampling, max_support)
+    g = Gridder(cfg.grid_n, wl["cell_rad"], cfg.n_wplanes, cfg.oversampling, max_support, cfg.n_pol)
+    g.allocate(None)
+    g.build_wkernels(wl["w_max"])
+    assert np.array_equal(g.supports, want), (g.supports, want)
+    assert want.max() > want.min()
+    wl = dict(wl, supports=want)
+    bank, off = orc.build_bank(want, wl["w_max"], wl["du"], cfg.oversampling, max_support)
+    ref = oracle_run(orc, wl, bank, off)
+    got_bank = g.debug_get_wkernels()
+    assert np.abs(got_bank.astype(np.complex128) - bank).max() <= 2e-7
+    uvw, bl, vis, wt = to_dev(torch_cuda, wl)
+    g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+    check_grid(g.grid_complex(), ref["grid"])
+    assert g.stats() == tuple(int(x) for x in ref["stats"])

@@ -123,3 +123,24 @@ def test_kernel_samples_agree_with_the_plane(orc):
         qv, qu = rng.integers(-20, 21, 50), rng.integers(-20, 21, 50)
         got = orc.kernel_samples(p, P, w_max, du, beta, n, qv, qu)
         assert np.abs(got - C[qv + 20, qu + 20]).max() < 1e-13
+
+
+def test_auto_supports_against_the_whole_plane(orc):
+    """Automatic supports (:1114 1e-3 rule, reading 7) pinned against the whole oversampled plane computed the
+    other way (E f E^T): outside the detected window the axis samples are <= 1e-3, the window is minimal, the
+    w = 0 plane of the spheroidal taper needs 7 cells, and supports do not shrink as |w| grows."""
+    P, w_max, du, beta, max_support = 6, 3000.0, 25.0, 4, 31
+    sup = orc.auto_supports(P, w_max, du, beta, max_support)
+    assert sup[0] == 7
+    assert (np.diff(sup) >= 0).all() and sup[-1] > sup[0]
+    assert (sup % 2 == 1).all() and sup.max() <= max_support
+    n = orc.inner_samples(max_support)
+    qmax = beta * ((max_support - 1) // 2)
+    for p in range(P):
+        C = np.abs(orc.oversampled_kernel(p, P, w_max, du, beta, n, -qmax, qmax))
+        axis = np.maximum(C[qmax, :], C[:, qmax])          # row and column through the centre
+        q = np.abs(np.arange(-qmax, qmax + 1))
+        h = (sup[p] - 1) // 2
+        if sup[p] < max_support:
+            assert axis[q > h * beta].max(initial=0.0) <= 1e-3
+        assert axis[q > (h - 1) * beta].max() > 1e-3        # one cell less would cut a sample above the threshold
