@@ -374,3 +374,15 @@ def test_automatic_supports_match_oracle_and_grid(orc, torch_cuda):
     g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
     check_grid(g.grid_complex(), ref["grid"])
     assert g.stats() == tuple(int(x) for x in ref["stats"])
+
+
+@pytest.mark.parametrize("idx", [2, 3])
+def test_full_size_config3_config4_sampled_pixels(idx, orc, torch_cuda):
+    """Same check on configs[2] and configs[3] at full size. Several minutes each on the host side (oracle indices of
+    266 M records), so they run only when IG_TEST_FULLSIZE_ALL=1; the result of the last run is recorded in
+    profiles/r01_fullsize_parity.md."""
+    import os
+    if os.environ.get("IG_TEST_FULLSIZE_ALL") != "1":
+        pytest.skip("set IG_TEST_FULLSIZE_ALL=1 to run the full-size checks of configs 3 and 4")
+    worst = _sampled_pixel_check(orc, torch_cuda, idx, n_pixels=3, seed=30 + idx)
+    print(f"config {idx + 1}: worst relative error over the sampled pixels {worst:.3e}")
