@@ -56,6 +56,21 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def ncu_traffic(config):
+    """DRAM bytes per launch of k_gridder from the committed ncu capture of this configuration
+    (profiles/traffic.csv: config,kernel,dram_read_bytes,dram_write_bytes,capture), or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        with open(path) as f:
+            for line in f:
+                c = [x.strip() for x in line.split(",")]
+                if len(c) >= 4 and c[0] == str(config) and c[1] == "k_gridder":
+                    return float(c[2]) + float(c[3])
+    except OSError:
+        pass
+    return None
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -285,10 +300,10 @@ def run_ours(args):
     gs = gridder_ms * 1e-3
     if t_byte >= t_flop:
         roof = {"bound": "hbm", "achieved": alg_bytes / gs / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                "frac": t_byte / gs, "traffic": None, "peak_source": peak_src}
+                "frac": t_byte / gs, "traffic": ncu_traffic(args.config), "peak_source": peak_src}
     else:
         roof = {"bound": "alu", "achieved": flops / gs / 1e12, "peak": fp32_peak, "unit": "TFLOP/s",
-                "frac": t_flop / gs, "traffic": None, "peak_source": "measured live: ig_measure_fp32_peak (FFMA loop)"}
+                "frac": t_flop / gs, "traffic": ncu_traffic(args.config), "peak_source": "measured live: ig_measure_fp32_peak (FFMA loop)"}
     roof.update({"kernel": "k_gridder", "kernel_ms": gridder_ms, "t_flop_ms": t_flop * 1e3, "t_byte_ms": t_byte * 1e3,
                  "algorithmic_bytes": int(alg_bytes), "flops": flops, "fp32_peak_tflops": fp32_peak, "hbm_peak_gbs": hbm_peak,
                  "commits": commits, "touched_pixels": touched})
