@@ -22,6 +22,8 @@ def torch_cuda():
     import torch
     if not torch.cuda.is_available():
         pytest.fail("gpu-marked test needs a CUDA device; there is no CPU fallback")
+    from paper_1403_4209_b200 import build
+    build.build()                      # no-op when libig.so is newer than its sources
     return torch
 
 
