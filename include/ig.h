@@ -135,6 +135,12 @@ ig_status ig_grid_host(ig_ctx* ctx, const double* uvw_m, const int* baseline_id,
  * Uses work_dev (ig_finalize_workspace_bytes()). Synchronises. */
 ig_status ig_finalize(ig_ctx* ctx, float* image_dev, double* normaliser_host);
 
+/* One grid per channel (the thesis's default mode, :1011, :1120; reading 16): with the switch on, grid_dev holds nchan
+ * grids back to back (each ig_grid_bytes(), same layout), channel c of every ig_grid call goes to grid c with its own
+ * normaliser, and ig_finalize_channel images one of them. Up to 4096 channels. Switch it before the first ig_grid. */
+ig_status ig_set_per_channel_grids(ig_ctx* ctx, int on);
+ig_status ig_finalize_channel(ig_ctx* ctx, int channel, float* image_dev, double* normaliser_host);
+
 /* eq 4.17: records gridded, records dropped, grid-point updates = sum S^2 * n_pol.
  * Cumulative over ig_grid calls. Synchronises. Any pointer may be NULL. */
 ig_status ig_get_stats(ig_ctx* ctx, long long* n_gridded, long long* n_dropped, long long* n_updates);

@@ -36,6 +36,8 @@ SIGNATURES = {
     "ig_set_host_slices": (_i, [_vp, _i]),
     "ig_grid_host": (_i, [_vp, _vp, _vp, _ll, _vp, _i, _vp, _vp]),
     "ig_finalize": (_i, [_vp, _vp, _vp]),
+    "ig_set_per_channel_grids": (_i, [_vp, _i]),
+    "ig_finalize_channel": (_i, [_vp, _i, _vp, _vp]),
     "ig_get_stats": (_i, [_vp, C.POINTER(_ll), C.POINTER(_ll), C.POINTER(_ll)]),
     "ig_get_commits": (_i, [_vp, C.POINTER(_ll)]),
     "ig_set_compression": (_i, [_vp, _i]),
@@ -125,20 +127,43 @@ class Gridder:
                                      _vp(self.work.data_ptr()), self.work.numel(),
                                      _vp(self.bank.data_ptr()), self.bank.numel(), self._stream_ptr()), "ig_bind")
 
-    def allocate(self, supports, work_bytes=0):
-        """Allocate grid (zeroed), bank and a work buffer of at least `work_bytes`."""
+    def allocate(self, supports, work_bytes=0, n_channel_grids=0):
+        """Allocate grid (zeroed), bank and a work buffer of at least `work_bytes`.
+        n_channel_grids > 0: one grid per channel (ig_set_per_channel_grids)."""
         t = self.torch
         if supports is not None:
             supports = np.ascontiguousarray(supports, dtype=np.int32)
             assert supports.size == self.n_wplanes
         self.supports = supports          # None: automatic supports, known after build_wkernels
         with t.cuda.device(self.device):
-            self.grid = t.zeros((self.grid_n, self.grid_n, self.n_pol, 2), dtype=t.float32, device=self.device)
+            shape = (self.grid_n, self.grid_n, self.n_pol, 2)
+            self.n_channel_grids = int(n_channel_grids)
+            if self.n_channel_grids > 0:
+                shape = (self.n_channel_grids,) + shape
+            self.grid = t.zeros(shape, dtype=t.float32, device=self.device)
             nb = self.lib.ig_bank_bytes(self.ctx, _np_ptr(supports) if supports is not None else None)
             self.bank = t.empty(nb, dtype=t.uint8, device=self.device)
             need = max(int(work_bytes), self.lib.ig_workspace_bytes(self.ctx, 0, 1), 1 << 20)
             self.work = t.empty(need, dtype=t.uint8, device=self.device)
         self._bind()
+        if self.n_channel_grids > 0:
+            self._check(self.lib.ig_set_per_channel_grids(self.ctx, 1), "ig_set_per_channel_grids")
+
+    def finalize_channel(self, channel):
+        t = self.torch
+        self.ensure_work(self.lib.ig_finalize_workspace_bytes(self.ctx))
+        img = t.empty((self.n_pol, self.grid_n, self.grid_n), dtype=t.float32, device=self.device)
+        norm = np.zeros(self.n_pol, dtype=np.float64)
+        self._check(self.lib.ig_finalize_channel(self.ctx, int(channel), _vp(img.data_ptr()), _np_ptr(norm)), "ig_finalize_channel")
+        return img, norm
+
+    def channel_grid_complex(self, channel) -> np.ndarray:
+        """Grid of one channel as complex64 numpy [N][N][npol] (per-channel grid mode)."""
+        self.torch.cuda.synchronize(self.device)
+        g, n = self.grid[channel], self.grid_n
+        if self.n_pol == 4:
+            g = g.reshape(2, n, n, 2, 2).permute(1, 2, 0, 3, 4).reshape(n, n, 4, 2)
+        return g.contiguous().cpu().numpy().view(np.complex64)[..., 0]
 
     def ensure_work(self, nbytes):
         if self.work is None or self.work.numel() < nbytes:

@@ -6,10 +6,11 @@
 namespace {
 ig_status fail(ig_ctx* c, ig_status s, const std::string& m) { if (c) c->err = m; return s; }
 
-// layout of bank_dev: [IgAccum][planes P][zeta P*beta^2][K data]
+// layout of bank_dev: [IgAccum][per-channel normalisers][planes P][zeta P*beta^2][K data]
 size_t bank_head_bytes(const ig_ctx* c) {
     size_t b2 = (size_t)c->prm.beta * c->prm.beta;
-    return ig_align(sizeof(IgAccum)) + ig_align((size_t)c->prm.P * sizeof(IgPlaneEntry)) + ig_align((size_t)c->prm.P * b2 * 8);
+    return ig_align(sizeof(IgAccum)) + ig_align((size_t)IG_MAX_CHAN_GRIDS * 4 * 8) + ig_align((size_t)c->prm.P * sizeof(IgPlaneEntry)) +
+           ig_align((size_t)c->prm.P * b2 * 8);
 }
 size_t bank_elems_of(const ig_ctx* c, const int* table) {
     size_t b2 = (size_t)c->prm.beta * c->prm.beta, e = 0;
@@ -128,12 +129,13 @@ ig_status ig_bind(ig_ctx* c, void* grid_dev, size_t grid_bytes, void* work_dev, 
     c->stream = (cudaStream_t)cuda_stream;
     char* p = c->bank_buf;
     c->d_acc = (IgAccum*)p; p += ig_align(sizeof(IgAccum));
+    c->d_chan_norm = (double*)p; p += ig_align((size_t)IG_MAX_CHAN_GRIDS * 4 * 8);
     c->d_planes = (IgPlaneEntry*)p; p += ig_align((size_t)c->prm.P * sizeof(IgPlaneEntry));
     c->d_zeta = (double*)p; p += ig_align((size_t)c->prm.P * c->prm.beta * c->prm.beta * 8);
     c->d_bank = (float2*)p;
     if (moved) {
         c->have_bank = false;
-        cudaError_t e = cudaMemsetAsync(c->d_acc, 0, sizeof(IgAccum), c->stream);
+        cudaError_t e = cudaMemsetAsync(c->d_acc, 0, ig_align(sizeof(IgAccum)) + (size_t)IG_MAX_CHAN_GRIDS * 4 * 8, c->stream);
         if (e != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_bind: ") + cudaGetErrorString(e));
     }
     for (auto& t : c->ev)
@@ -210,6 +212,8 @@ ig_status ig_grid(ig_ctx* c, const double* uvw, const int* baseline_id, long lon
     if (!c) return IG_EINVAL;
     if (!c->bound || !c->have_bank) return fail(c, IG_ESTATE, "ig_bind and ig_build_wkernels first");
     if (nrow < 0 || nchan < 1 || !freqs) return fail(c, IG_EINVAL, "bad nrow/nchan/freqs");
+    if (c->per_channel && (nchan > IG_MAX_CHAN_GRIDS || (size_t)nchan * ig_grid_bytes(c) > c->grid_bytes))
+        return fail(c, IG_ENOMEM, "per-channel grids: the bound grid buffer holds fewer than nchan grids");
     c->launches = 0;
     if (nrow == 0) return IG_OK;
     if (!uvw || !baseline_id || !vis || !wt) return fail(c, IG_EINVAL, "null input");
@@ -309,10 +313,26 @@ ig_status ig_grid_host(ig_ctx* c, const double* uvw, const int* baseline_id, lon
     return IG_OK;
 }
 
+ig_status ig_set_per_channel_grids(ig_ctx* c, int on) {
+    if (!c) return IG_EINVAL;
+    c->per_channel = on != 0;
+    return IG_OK;
+}
+
+ig_status ig_finalize_channel(ig_ctx* c, int channel, float* image_dev, double* norm_host) {
+    if (!c || !image_dev || channel < 0 || channel >= IG_MAX_CHAN_GRIDS) return IG_EINVAL;
+    if (!c->bound || !c->have_bank || !c->per_channel) return fail(c, IG_ESTATE, "per-channel grids are not in use");
+    if ((size_t)(channel + 1) * ig_grid_bytes(c) > c->grid_bytes) return fail(c, IG_EINVAL, "no such channel grid");
+    int r = ig_run_finalize(c, channel, image_dev, norm_host);
+    if (r == -2) return IG_ENOMEM;
+    return r < 0 ? IG_ECUDA : IG_OK;
+}
+
 ig_status ig_finalize(ig_ctx* c, float* image_dev, double* norm_host) {
     if (!c || !image_dev) return IG_EINVAL;
     if (!c->bound || !c->have_bank) return fail(c, IG_ESTATE, "nothing to finalise");
-    int r = ig_run_finalize(c, image_dev, norm_host);
+    if (c->per_channel) return fail(c, IG_ESTATE, "per-channel grids: use ig_finalize_channel");
+    int r = ig_run_finalize(c, -1, image_dev, norm_host);
     if (r == -2) return IG_ENOMEM;
     return r < 0 ? IG_ECUDA : IG_OK;
 }
@@ -380,7 +400,7 @@ ig_status ig_get_timing(ig_ctx* c, int calls_back, float* ingest_ms, float* grid
 ig_status ig_reset_accumulators(ig_ctx* c) {
     if (!c) return IG_EINVAL;
     if (!c->bound) return fail(c, IG_ESTATE, "ig_bind first");
-    if (cudaMemsetAsync(c->d_acc, 0, sizeof(IgAccum), c->stream) != cudaSuccess) return fail(c, IG_ECUDA, "memset failed");
+    if (cudaMemsetAsync(c->d_acc, 0, ig_align(sizeof(IgAccum)) + (size_t)IG_MAX_CHAN_GRIDS * 4 * 8, c->stream) != cudaSuccess) return fail(c, IG_ECUDA, "memset failed");
     return IG_OK;
 }
 

@@ -41,12 +41,18 @@ size_t ig_finalize_scratch_bytes(const ig_ctx* c) {
     return ig_align(N * N * 8) + ig_align(N * 8) + ig_align(fft_work_bytes((int)N));
 }
 
-int ig_run_finalize(ig_ctx* c, float* image, double* norm_host) {
+int ig_run_finalize(ig_ctx* c, int channel, float* image, double* norm_host) {
     const int N = c->prm.N, npol = c->prm.npol;
     if (c->work_bytes < ig_finalize_scratch_bytes(c)) { c->err = "work buffer too small for ig_finalize"; return -2; }
     IgAccum acc;
     IG_CUDA_OK(c, cudaMemcpyAsync(&acc, c->d_acc, sizeof(acc), cudaMemcpyDeviceToHost, c->stream));
     IG_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    const float2* grid = (const float2*)c->grid;
+    if (channel >= 0) {                 // one grid per channel: its own grid and normaliser
+        grid += (size_t)channel * N * N * npol;
+        IG_CUDA_OK(c, cudaMemcpyAsync(acc.norm, c->d_chan_norm + (size_t)channel * 4, 4 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        IG_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    }
     if (norm_host) for (int q = 0; q < npol; ++q) norm_host[q] = acc.norm[q];
 
     float2* plane = (float2*)c->work;
@@ -75,9 +81,9 @@ int ig_run_finalize(ig_ctx* c, float* image, double* norm_host) {
     dim3 g((N + 255) / 256, N), b(256);
     for (int q = 0; q < npol; ++q) {
         switch (npol) {
-            case 1: k_fin_extract<1><<<g, b, 0, c->stream>>>((const float2*)c->grid, plane, N, q); break;
-            case 2: k_fin_extract<2><<<g, b, 0, c->stream>>>((const float2*)c->grid, plane, N, q); break;
-            default: k_fin_extract<4><<<g, b, 0, c->stream>>>((const float2*)c->grid, plane, N, q); break;
+            case 1: k_fin_extract<1><<<g, b, 0, c->stream>>>(grid, plane, N, q); break;
+            case 2: k_fin_extract<2><<<g, b, 0, c->stream>>>(grid, plane, N, q); break;
+            default: k_fin_extract<4><<<g, b, 0, c->stream>>>(grid, plane, N, q); break;
         }
         if (cufftExecC2C(plan, (cufftComplex*)plane, (cufftComplex*)plane, CUFFT_INVERSE) != CUFFT_SUCCESS) {
             cufftDestroy(plan); c->err = "cufftExecC2C failed"; return -1;

@@ -225,7 +225,7 @@ template <int NPOL, bool COUNT>
 __global__ void __launch_bounds__(IG_GRID_WARPS * 32, IG_GRID_CTAS_PER_SM)
 k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_smax, unsigned nrb, unsigned nchan,
           float* __restrict__ grid, const float2* __restrict__ bank, int N, unsigned* __restrict__ ticket,
-          unsigned long long* __restrict__ commits) {
+          unsigned long long* __restrict__ commits, size_t chan_stride) {
     constexpr int STRIDE = NPOL == 4 ? 48 : 32;
     constexpr int STAGE_BYTES = IG_STAGE * STRIDE;
     __shared__ __align__(128) char sm_rec[IG_GRID_WARPS][IG_CH * STRIDE];
@@ -252,6 +252,7 @@ k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_s
         // tickets run channel-major: neighbours in the queue are neighbouring row blocks of ONE channel
         const unsigned ch = tk / nrb;
         const unsigned chunk = (tk - ch * nrb) * nchan + ch;
+        float* __restrict__ grid_ch = grid + (size_t)ch * chan_stride;   // per-channel grids: chan_stride = floats per grid, else 0
         if (chunk_smax[chunk] == 0) continue;          // every record of the item was dropped
         __syncwarp();                                  // all lanes are done with the previous item
         if (lane == 0) {
@@ -297,7 +298,7 @@ k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_s
                 for (int pass = 0; pass < n_pass; ++pass) {
                     const int q0 = pass * 32 * R + lane;
                     switch (R) {
-#define IG_CASE(r) case r: n_commit += grid_run<NPOL, r, COUNT>(rp, r1 - r0, S, q0, grid, bank, N); break;
+#define IG_CASE(r) case r: n_commit += grid_run<NPOL, r, COUNT>(rp, r1 - r0, S, q0, grid_ch, bank, N); break;
                         IG_CASE(1) IG_CASE(2)
 #if IG_RMAX >= 3
                         IG_CASE(3)
@@ -341,7 +342,7 @@ int ig_launch_gridder(ig_ctx* c, const char* records, const uint32_t* chunk_smax
     long long want = (n_chunks + IG_GRID_WARPS - 1) / IG_GRID_WARPS;
     unsigned ctas = (unsigned)(want < (long long)sms * per_sm ? want : (long long)sms * per_sm);
     dim3 g(ctas), b(IG_GRID_WARPS * 32);
-#define IG_LAUNCH(P, C) k_gridder<P, C><<<g, b, 0, c->stream>>>(records, chunk_smax, (unsigned)nrb, (unsigned)nchan, c->grid, c->d_bank, c->prm.N, &c->d_acc->ticket, &c->d_acc->commits)
+#define IG_LAUNCH(P, C) k_gridder<P, C><<<g, b, 0, c->stream>>>(records, chunk_smax, (unsigned)nrb, (unsigned)nchan, c->grid, c->d_bank, c->prm.N, &c->d_acc->ticket, &c->d_acc->commits, c->per_channel ? (size_t)c->prm.N * c->prm.N * c->prm.npol * 2 : (size_t)0)
     if (c->count_commits) {
         switch (c->prm.npol) { case 1: IG_LAUNCH(1, true); break; case 2: IG_LAUNCH(2, true); break; default: IG_LAUNCH(4, true); break; }
     } else {

@@ -73,7 +73,7 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
         const double* __restrict__ uvw, const uint32_t* __restrict__ perm, long long nrow,
         const double* __restrict__ freqs, int nchan, const float* __restrict__ vis,
         const float* __restrict__ wt, char* __restrict__ records, uint32_t* __restrict__ chunk_smax,
-        IgAccum* __restrict__ acc, bool compress) {
+        IgAccum* __restrict__ acc, bool compress, double* __restrict__ chan_norm) {
     constexpr int STRIDE = NPOL == 4 ? 48 : 32;
     const long long rb = blockIdx.x;
     const int t = threadIdx.x, lane = t & 31;
@@ -101,6 +101,9 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
 #pragma unroll
         for (int q = 0; q < 2 * NPOL; ++q) v[q] = 0.f;
         int S = 0;
+        double cn[NPOL];                  // this record's normaliser terms (per-channel grid mode)
+#pragma unroll
+        for (int q = 0; q < NPOL; ++q) cn[q] = 0.0;
         if (live) {
             IgIndex ix = ig_index_one(P, planes, um, vm, wm, freqs[c]);
             const float* vp = vis + ((size_t)row * nchan + c) * (2 * NPOL);
@@ -132,7 +135,8 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
                 const double z = zeta[(size_t)ix.p * P.beta * P.beta + tab];
 #pragma unroll
                 for (int q = 0; q < NPOL; ++q) {
-                    nsum[q] += (double)w[q] * z;              // eq 4.5
+                    cn[q] = (double)w[q] * z;
+                    nsum[q] += cn[q];                         // eq 4.5
                     v[2 * q] = w[q] * v[2 * q];               // eq 4.16
                     v[2 * q + 1] = conj ? -(w[q] * v[2 * q + 1]) : w[q] * v[2 * q + 1];
                 }
@@ -178,6 +182,15 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
             *reinterpret_cast<float4*>(rec + 16) = make_float4(v[0], v[1], v[2], v[3]);
         } else {
             *reinterpret_cast<float4*>(rec + 16) = make_float4(v[0], v[1], 0.f, 0.f);
+        }
+        if (chan_norm) {                  // one grid per channel: eq 4.5 per channel
+#pragma unroll
+            for (int q = 0; q < NPOL; ++q) {
+                double x = cn[q];
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+                if (lane == 0 && x != 0.0) atomicAdd(&chan_norm[(size_t)c * 4 + q], x);
+            }
         }
         unsigned smax = __reduce_max_sync(0xffffffffu, (unsigned)S);
         if (lane == 0 && smax) atomicMax(&chunk_smax[chunk], smax);
@@ -234,9 +247,9 @@ int ig_launch_index(ig_ctx* c, const double* uvw, const uint32_t* perm, long lon
     IG_CUDA_OK(c, cudaMemsetAsync(chunk_smax, 0, (size_t)nrb * nchan * 4, c->stream));
     dim3 g((unsigned)nrb), b(IG_CH);
     switch (c->prm.npol) {
-        case 1: k_index<1><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc, c->compress); break;
-        case 2: k_index<2><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc, c->compress); break;
-        default: k_index<4><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc, c->compress); break;
+        case 1: k_index<1><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc, c->compress, c->per_channel ? c->d_chan_norm : nullptr); break;
+        case 2: k_index<2><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc, c->compress, c->per_channel ? c->d_chan_norm : nullptr); break;
+        default: k_index<4><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc, c->compress, c->per_channel ? c->d_chan_norm : nullptr); break;
     }
     IG_CUDA_OK(c, cudaGetLastError());
     return 1;

@@ -19,6 +19,7 @@
 #endif
 // IG_GRID_CTAS_PER_SM: launch bound and persistent grid size
 #define IG_HDR_MERGED (1u << 25)   // record header word z: visibility already summed into the run's head record
+#define IG_MAX_CHAN_GRIDS 4096   // per-channel grid mode: channels whose normalisers the bank head has room for
 #define IG_GRID_WARPS 4      // warps per gridder CTA
 
 // Device-side tail of the bank buffer: small tables and accumulators.
@@ -51,6 +52,8 @@ struct ig_ctx {
     int host_slices = 8;                      // ig_set_host_slices
     cudaStream_t copy_stream = nullptr;       // ig_grid_host: H2D copies of the next slice
     cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
+    bool per_channel = false;                 // ig_set_per_channel_grids: one grid per channel (thesis default, :1120)
+    double* d_chan_norm = nullptr;            // [IG_MAX_CHAN_GRIDS][4] normalisers of the per-channel grids
     bool compress = true;                     // ig_set_compression
     bool count_commits = false;               // ig_set_commit_counting
     // bank description (host copies)
@@ -80,7 +83,7 @@ size_t ig_sort_scratch_bytes(long long nrow);
 // (compression is applied in k_index when c->compress is set)
 int ig_launch_index(ig_ctx* c, const double* uvw, const uint32_t* perm, long long nrow,
                     const double* d_freqs, int nchan, const float* vis, const float* wt,
-                    char* records, uint32_t* chunk_smax);
+                    char* records, uint32_t* chunk_smax);   // uses c->per_channel / c->d_chan_norm
 int ig_launch_debug_index(ig_ctx* c, const double* uvw, long long nrow, const double* d_freqs, int nchan,
                           int* X, int* Y, int* ou, int* ov, int* pl, int* fl);
 int ig_launch_gridder(ig_ctx* c, const char* records, const uint32_t* chunk_smax, long long nrb, int nchan);
@@ -88,7 +91,7 @@ int ig_launch_bank(ig_ctx* c, char* scratch, size_t scratch_bytes);
 size_t ig_bank_scratch_bytes(const ig_ctx* c);
 int ig_launch_zeta(ig_ctx* c);
 int ig_detect_supports(ig_ctx* c, char* scratch, size_t scratch_bytes, int* table);
-int ig_run_finalize(ig_ctx* c, float* image, double* norm_host);
+int ig_run_finalize(ig_ctx* c, int channel, float* image, double* norm_host);   // channel < 0: the single grid
 size_t ig_finalize_scratch_bytes(const ig_ctx* c);
 
 #define IG_CUDA_OK(ctx, call)                                                        \

@@ -43,7 +43,7 @@ def test_create_validates_arguments(lib):
     assert lib.ig_grid_bytes(ctx) == 256 * 256 * 4 * 8
     sup = np.array([7, 7, 5, 3], dtype=np.int32)
     head = lib.ig_bank_bytes(ctx, sup.ctypes.data_as(ctypes.c_void_p)) - (49 + 49 + 25 + 9) * 64 * 8
-    assert 0 < head < 8192
+    assert 0 < head < 8192 + 4096 * 4 * 8 + 256      # accumulators, per-channel normalisers, plane table, zeta
     assert lib.ig_bank_bytes(ctx, None) >= lib.ig_bank_bytes(ctx, sup.ctypes.data_as(ctypes.c_void_p))
     w1, w2 = lib.ig_workspace_bytes(ctx, 1000, 4), lib.ig_workspace_bytes(ctx, 100000, 4)
     assert w2 > w1 > 0

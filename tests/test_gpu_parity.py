@@ -388,3 +388,35 @@ def test_full_size_config3_config4_sampled_pixels(idx, orc, torch_cuda):
         pytest.skip("set IG_TEST_FULLSIZE_ALL=1 to run the full-size checks of configs 3 and 4")
     worst = _sampled_pixel_check(orc, torch_cuda, idx, n_pixels=3, seed=30 + idx)
     print(f"config {idx + 1}: worst relative error over the sampled pixels {worst:.3e}")
+
+
+def test_per_channel_grids(orc, torch_cuda):
+    """One grid per channel (the thesis's default, :1120): channel c of the batch goes to grid c with its own
+    normaliser; each equals the oracle run on that channel alone; ig_finalize_channel images it."""
+    from paper_1403_4209_b200.binding import Gridder, IgError
+    cfg = small(synth.CONFIGS[1], n_station=9, n_time=150, n_chan=3, n_wplanes=8)
+    wl = synth.make_workload(cfg)
+    sup = wl["supports"]
+    bank, off = orc.build_bank(sup, wl["w_max"], wl["du"], cfg.oversampling, int(sup.max()))
+    g = Gridder(cfg.grid_n, wl["cell_rad"], cfg.n_wplanes, cfg.oversampling, int(sup.max()), cfg.n_pol)
+    g.allocate(sup, n_channel_grids=cfg.n_chan)
+    g.debug_set_wkernels(wl["w_max"], bank.astype(np.complex64))
+    uvw, bl, vis, wt = to_dev(torch_cuda, wl)
+    g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+    with pytest.raises(IgError):
+        g.finalize()                                   # the single-grid finaliser refuses in this mode
+    total = np.zeros(3, dtype=np.int64)
+    for c in range(cfg.n_chan):
+        one = dict(wl, freqs_hz=wl["freqs_hz"][c:c + 1], vis=np.ascontiguousarray(wl["vis"][:, c:c + 1]),
+                   weights=np.ascontiguousarray(wl["weights"][:, c:c + 1]))
+        ref = oracle_run(orc, one, bank, off)
+        check_grid(g.channel_grid_complex(c), ref["grid"])
+        img, norm = g.finalize_channel(c)
+        assert np.allclose(norm, ref["norm"], rtol=1e-6, atol=0)
+        want = orc.finalize(ref["grid"], ref["norm"], cfg.oversampling)
+        n = cfg.grid_n
+        inner = slice(n // 8, n - n // 8)
+        got = img.cpu().numpy().astype(np.float64)
+        assert np.abs(got[:, inner, inner] - want[:, inner, inner]).max() <= 2e-4 * np.abs(want[:, inner, inner]).max()
+        total += ref["stats"]
+    assert g.stats() == tuple(int(x) for x in total)
