@@ -93,7 +93,26 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
     for (int q = 0; q < NPOL; ++q) nsum[q] = 0.0;
     unsigned long long n_grid = 0, n_drop = 0, n_upd = 0, n_merged = 0;
 
-    for (int c = 0; c < nchan; ++c) {
+    // Channels are taken four at a time and their visibilities and weights requested together: a row's four
+    // channels are one 128-byte line (4 pol), so DRAM sees whole lines instead of four separate sector reads.
+    constexpr int CG = 4;
+    for (int c0 = 0; c0 < nchan; c0 += CG) {
+      float4 pre_a[CG], pre_b[CG], pre_w[CG];
+      if constexpr (NPOL == 4) {
+#pragma unroll
+          for (int k = 0; k < CG; ++k) {
+              if (live && c0 + k < nchan) {
+                  const float* vp = vis + ((size_t)row * nchan + c0 + k) * 8;
+                  pre_a[k] = *reinterpret_cast<const float4*>(vp);
+                  pre_b[k] = *reinterpret_cast<const float4*>(vp + 4);
+                  pre_w[k] = *reinterpret_cast<const float4*>(wt + ((size_t)row * nchan + c0 + k) * 4);
+              }
+          }
+      }
+#pragma unroll
+      for (int k = 0; k < CG; ++k) {
+        const int c = c0 + k;
+        if (c >= nchan) break;
         const long long chunk = rb * nchan + c;
         char* rec = records + ((size_t)chunk * IG_CH + t) * STRIDE;
         uint4 hdr = make_uint4(0u, 0u, 0u, 0u);
@@ -111,9 +130,10 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
             float w[NPOL];
             bool any = false;
             if constexpr (NPOL == 4) {
-                float4 w4 = *reinterpret_cast<const float4*>(wp);
+                const float4 w4 = pre_w[k];
                 w[0] = w4.x; w[1] = w4.y; w[2] = w4.z; w[3] = w4.w;
-                float4 a = *reinterpret_cast<const float4*>(vp), b = *reinterpret_cast<const float4*>(vp + 4);
+                const float4 a = pre_a[k], b = pre_b[k];
+                (void)vp; (void)wp;
                 v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
             } else {
 #pragma unroll
@@ -194,6 +214,7 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
         }
         unsigned smax = __reduce_max_sync(0xffffffffu, (unsigned)S);
         if (lane == 0 && smax) atomicMax(&chunk_smax[chunk], smax);
+      }
     }
 
     // block reduction of the normaliser and the counters
