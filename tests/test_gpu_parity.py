@@ -420,3 +420,36 @@ def test_per_channel_grids(orc, torch_cuda):
         assert np.abs(got[:, inner, inner] - want[:, inner, inner]).max() <= 2e-4 * np.abs(want[:, inner, inner]).max()
         total += ref["stats"]
     assert g.stats() == tuple(int(x) for x in total)
+
+
+def test_buffers_are_not_overrun(runs, torch_cuda):
+    """Guard bytes around the caller's grid, work and bank buffers survive build + ig_grid + ig_finalize
+    (compute-sanitizer is closed on this pool, so the bounds are checked this way): the buffers are bound at
+    exactly the sizes the size queries return."""
+    t = torch_cuda
+    wl, ref = runs("cfg3s")
+    cfg = wl["cfg"]
+    g = make_gridder(wl)
+    G = 4096
+    uvw, bl, vis, wt = to_dev(t, wl)
+    nrow = uvw.shape[0]
+    need_work = max(g.workspace_bytes(nrow, cfg.n_chan), g.lib.ig_finalize_workspace_bytes(g.ctx),
+                    g.lib.ig_workspace_bytes(g.ctx, 0, 1))
+    need_bank = g.bank.numel()
+    need_grid = g.grid.numel() * 4
+    bufs = {}
+    for name, need in (("work", need_work), ("bank", need_bank), ("grid", need_grid)):
+        big = t.full((need + 2 * G,), 0xAB, dtype=t.uint8, device="cuda:0")
+        big[G:G + need] = 0
+        bufs[name] = big
+    g.work = bufs["work"][G:G + need_work]
+    g.bank = bufs["bank"][G:G + need_bank]
+    g.grid = bufs["grid"][G:G + need_grid].view(t.float32).view(cfg.grid_n, cfg.grid_n, cfg.n_pol, 2)
+    g._bind()
+    g.build_wkernels(wl["w_max"])
+    g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+    check_grid(g.grid_complex(), ref["grid"])
+    g.finalize()
+    t.cuda.synchronize()
+    for name, big in bufs.items():
+        assert bool((big[:G] == 0xAB).all()) and bool((big[-G:] == 0xAB).all()), f"{name} buffer overrun"
