@@ -6,8 +6,8 @@
 // grid points whose coordinates are congruent to its (i,j) modulo the support S, keeps
 // their sums in registers while successive records of a track overlap, and commits a
 // point with an atomic only when the footprint has moved off it. What is new for sm_100a:
-//  - the unit is ONE WARP, not a thread block: a warp owns 32*R points (R <= 8 per lane),
-//    so a 9x9 footprint is one warp with R = 3 and a 129x129 one is 65 passes of R = 8;
+//  - the unit is ONE WARP, not a thread block: a warp owns 32*R points (R <= IG_RMAX = 4 per lane),
+//    so a 9x9 footprint is one pass with R = 3 and a 129x129 one is 131 passes of R = 4;
 //    the small supports that dominate W-projection workloads (and that the thesis's
 //    256/1024-thread blocks served badly, :1375,:1986) fill the lanes;
 //  - work items are fixed-size chunks of IG_CH records taken from a device-side ticket
