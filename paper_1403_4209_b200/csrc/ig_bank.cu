@@ -275,12 +275,10 @@ int ig_detect_supports(ig_ctx* c, char* scratch, size_t scratch_bytes, int* tabl
 int ig_launch_bank(ig_ctx* c, char* scratch, size_t scratch_bytes) {
     if (scratch_bytes < ig_bank_scratch_bytes(c)) { c->err = "work buffer too small for the bank builder"; return -1; }
     const int n = bank_inner_samples(c->max_support), beta = c->prm.beta, M = n * beta;
-    const size_t Qmax = (size_t)c->max_support * beta;
     double* d_psi = (double*)scratch;
     double2* d_W = (double2*)(scratch + ig_align((size_t)n * 8));
     double2* d_f = (double2*)((char*)d_W + ig_align((size_t)M * 16));
     double2* d_G = (double2*)((char*)d_f + ig_align((size_t)n * n * 16));
-    (void)Qmax;
     std::vector<double> eta(n), psi(n);
     for (int i = 0; i < n; ++i) eta[i] = 2.0 * (double)(i - n / 2) / (double)n;
     ig_taper_eval(eta.data(), n, psi.data());

@@ -30,7 +30,7 @@ struct IgAccum {
     unsigned long long merged;          // records pre-summed into their predecessor (compression)
     unsigned long long commits;         // pixel commits (atomic reductions of one multi-pol pixel) by the gridder
     unsigned int ticket;                // work queue of the gridder
-    unsigned int max_key;               // largest baseline id of the current call
+    unsigned int pad_;
 };
 
 struct IgParams {            // passed by value to kernels
@@ -73,7 +73,7 @@ struct ig_ctx {
 static inline size_t ig_align(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 static inline int ig_rec_stride(int npol) { return npol == 4 ? 48 : 32; }  // bytes, multiple of 16
 
-// ig_taper.cpp-ish (host, in ig_bank.cu)
+// the taper psi(eta), host code in ig_bank.cu
 void ig_taper_eval(const double* eta, int n, double* psi);
 
 // launchers (each returns the number of kernels launched, or -1 with ctx->err set)
