@@ -5,11 +5,13 @@ A "step" is one pass of the whole hot path (ingest A1-A3 + gridder C = one ig_gr
 full synthetic workload of the chosen BASELINE.json configuration. `value` = grid-point updates/s
 (sum S^2 * n_pol over gridded records / device time, sec 5.3.1) with inputs resident in
 HBM; `e2e` = the same through ig_grid_host with pinned host buffers, copies inside the timed region.
+`per_config` times the other BASELINE.json configurations in the same process (device-resident inputs).
 `--impl reference` times the fp64 CPU oracle (oracle/), as it stands, on a bounded sample.
 """
 from __future__ import annotations
 
 import argparse
+import gc
 import json
 import os
 import subprocess
@@ -41,9 +43,12 @@ def parse():
     ap.add_argument("--support-law", default="w", choices=["w", "k"])
     ap.add_argument("--no-compress", action="store_true", help="switch compression off (thesis: real vs total rate)")
     ap.add_argument("--host-slices", type=int, default=8, help="ig_grid_host: slices copied while the previous one is gridded")
+    ap.add_argument("--gather-min-support", type=int, default=None, help="ig_set_gather_min_support (experiments)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="time only --config (default: configs 1-4 too, after the main one)")
     ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--cpu-full", action="store_true", help="cpu_baseline: also time configs 1-3 in full (minutes)")
     return ap.parse_args()
 
 
@@ -57,16 +62,31 @@ def peaks():
 
 
 def ncu_traffic(config):
-    """DRAM bytes per launch of k_gridder from the committed ncu capture of this configuration
+    """DRAM bytes per launch of the gridder from the committed ncu capture of this configuration
     (profiles/traffic.csv: config,kernel,dram_read_bytes,dram_write_bytes,capture), or None."""
     path = os.path.join(ROOT, "profiles", "traffic.csv")
+    tot = None
     try:
         with open(path) as f:
             for line in f:
                 c = [x.strip() for x in line.split(",")]
-                if len(c) >= 4 and c[0] == str(config) and c[1] == "k_gridder":
-                    return float(c[2]) + float(c[3])
+                if len(c) >= 4 and c[0] == str(config) and c[1].startswith("k_g"):
+                    tot = (tot or 0.0) + float(c[2]) + float(c[3])
     except OSError:
+        pass
+    return tot
+
+
+def model_commits(config, law):
+    """Pixel commits of the track-order register-accumulation model, computed from the ORACLE's indices by
+    `python -m oracle.track_commits` and stored in oracle/track_commits.json (a plain data file: bench.py's
+    roofline must not depend on what the kernel under test happens to commit). None if not stored."""
+    try:
+        with open(os.path.join(ROOT, "oracle", "track_commits.json")) as f:
+            for e in json.load(f)["entries"]:
+                if e["config"] == WORKLOADS[config - 1] and e["support_law"] == law:
+                    return int(e["pixel_commits"])
+    except (OSError, KeyError, ValueError):
         pass
     return None
 
@@ -88,6 +108,7 @@ class ClockSampler:
             self.t.start()
         except Exception:
             self.proc = None
+        return self
 
     def _read(self):
         for line in self.proc.stdout:
@@ -118,22 +139,25 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def cpu_oracle_sample(cfg, law, target_s):
+# ---------------------------------------------------------------------------------------------------------
+# CPU oracle legs
+# ---------------------------------------------------------------------------------------------------------
+def cpu_oracle_sample(cfg, law, target_s, n_threads=0, full=False):
     """Time the oracle (index + gridding, fp64, OpenMP row bands) on the first whole time steps of the
-    workload. The kernel-bank VALUES are seeded random numbers of the right shape: the oracle's own numpy
-    bank builder would take minutes for hundreds of planes, and the record loop's work does not depend on
-    them. Returns dict(value, cores, sample, seconds, updates, records)."""
+    workload (`full`: on all of it). The kernel-bank VALUES are seeded random numbers of the right shape: the
+    oracle's own numpy bank builder would take minutes for hundreds of planes, and the record loop's work does
+    not depend on them. Returns dict(value, cores, sample, seconds, updates, records)."""
     from oracle import reference as orc
     orc.build()
     n_bl = cfg.n_station * (cfg.n_station - 1) // 2
     wl_full = synth.make_workload(cfg, law, with_vis=False)
     sup = wl_full["supports"]
     mean_s2 = float((sup.astype(np.float64) ** 2).mean())
-    # aim at target_s assuming ~2e8 fp64 complex updates/s/core as a first guess
-    cores = orc.threads()
-    guess_updates = 2e8 * cores * target_s
+    cores = orc.threads() if n_threads <= 0 else n_threads
+    orc.set_threads(cores)
+    guess_updates = 2e8 * cores * target_s          # first guess: ~2e8 fp64 complex updates/s/core
     per_step = n_bl * cfg.n_chan * mean_s2 * cfg.n_pol * 0.35
-    n_t = int(max(1, min(cfg.n_time, guess_updates // max(per_step, 1))))
+    n_t = cfg.n_time if full else int(max(1, min(cfg.n_time, guess_updates // max(per_step, 1))))
     rows = n_t * n_bl
     uvw, bl = wl_full["uvw_m"][:rows], wl_full["baseline"][:rows]
     rng = np.random.Generator(np.random.Philox(99))
@@ -152,10 +176,11 @@ def cpu_oracle_sample(cfg, law, target_s):
                             cfg.n_wplanes, wl_full["w_max"], sup)
     _, _, stats = orc.grid_records(idx, vis, wt, cfg.grid_n, cfg.oversampling, sup, bank, off, grid=grid)
     dt = time.perf_counter() - t0
+    orc.set_threads(orc.threads() if n_threads <= 0 else os.cpu_count() or 1)
     return dict(value=float(stats[2]) / dt, cores=cores, seconds=dt, updates=int(stats[2]), records=int(stats[0]),
-                sample=f"oracle orc_index+orc_grid (fp64, {cores} OpenMP threads) on the first {n_t} of {cfg.n_time} time "
-                       f"steps x all {n_bl} baselines x {cfg.n_chan} channels = {int(stats[0])} records of {cfg.name}; "
-                       f"kernel-bank values seeded random (timing only)")
+                sample=f"oracle orc_index+orc_grid (fp64, {cores} OpenMP thread{'s' if cores > 1 else ''}) on the first {n_t} of "
+                       f"{cfg.n_time} time steps x all {n_bl} baselines x {cfg.n_chan} channels = {int(stats[0])} records of "
+                       f"{cfg.name}; kernel-bank values seeded random (timing only)")
 
 
 def run_reference(args):
@@ -182,11 +207,169 @@ def run_reference(args):
     }))
 
 
+# ---------------------------------------------------------------------------------------------------------
+# GPU leg
+# ---------------------------------------------------------------------------------------------------------
+def roofline_of(config, law, cfg, sup, nrow, nchan, npol, updates, commits_measured, touched, gridder_ms, fp32_peak,
+                commit_rate_l2):
+    """The gridding roofline of north_star / SURVEY 8(d) for the gridder phase: the slower of 8 flops per complex
+    update at the measured FP32 peak and the algorithmic bytes at the measured HBM copy bandwidth. The atomic term
+    uses the ORACLE-derived track-order commit count (oracle/track_commits.json), not the kernel's own counter."""
+    hbm_peak, peak_src = peaks()
+    stride = 48 if npol == 4 else 32
+    n_chunks = ((nrow + 127) // 128) * nchan
+    bank_bytes = int((sup.astype(np.int64) ** 2).sum()) * cfg.oversampling ** 2 * 8
+    rec_bytes = n_chunks * 128 * stride
+    grid_bytes = touched * 8 * npol * 2
+    commits_model = model_commits(config, law)
+    commits = commits_model if commits_model is not None else commits_measured
+    compulsory = rec_bytes + bank_bytes + grid_bytes
+    alg_bytes = compulsory + commits * 8 * npol
+    t_byte = alg_bytes / (hbm_peak * 1e9)
+    flops = 8.0 * updates
+    t_flop = flops / (fp32_peak * 1e12)
+    gs = gridder_ms * 1e-3
+    traffic = ncu_traffic(config)
+    if t_byte >= t_flop:
+        roof = {"bound": "hbm", "achieved": alg_bytes / gs / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                "frac": t_byte / gs, "traffic": traffic, "peak_source": peak_src}
+    else:
+        roof = {"bound": "alu", "achieved": flops / gs / 1e12, "peak": fp32_peak, "unit": "TFLOP/s",
+                "frac": t_flop / gs, "traffic": traffic, "peak_source": "measured live: ig_measure_fp32_peak (FFMA loop)"}
+    roof.update({
+        "kernel": "gridder phase (k_gridder + k_gather, CUDA events around both)", "kernel_ms": gridder_ms,
+        "t_flop_ms": t_flop * 1e3, "t_byte_ms": t_byte * 1e3, "frac_alu": t_flop / gs, "frac_hbm_model": t_byte / gs,
+        "algorithmic_bytes": int(alg_bytes), "compulsory_hbm_bytes": int(compulsory),
+        "frac_compulsory_hbm": compulsory / (hbm_peak * 1e9) / gs,
+        "flops": flops, "fp32_peak_tflops": fp32_peak, "hbm_peak_gbs": hbm_peak,
+        "commits": commits, "commits_source": ("oracle/track_commits.json (track-order model from the oracle's indices)"
+                                                if commits_model is not None else "kernel counter (no stored model for this workload)"),
+        "commits_measured": commits_measured, "touched_pixels": touched,
+        "l2_commit_rate_gcommits_s": commit_rate_l2,
+        "t_atomic_l2_ms": (commits / (commit_rate_l2 * 1e9) * 1e3) if commit_rate_l2 else None,
+        "bytes_model": "records 48 B + bank once + model commits x 8 B x n_pol + touched pixels x 8 B x n_pol x 2 (DESIGN.md section 5)"})
+    return roof
+
+
+def bench_config(args, config, dev, ranks, steps, warmup, want_e2e, fp32_peak, commit_rate_l2, sample_clocks):
+    """Generates the workload of one configuration, grids it warmup + steps times, returns the measurements."""
+    import torch
+    from paper_1403_4209_b200.binding import Gridder
+    world, rank = ranks.world, ranks.rank
+    cfg = synth.CONFIGS[config - 1]
+    t_gen = time.perf_counter()
+    wl = synth.make_workload(cfg, args.support_law)       # replicas only: every rank grids the same workload
+    t_gen = time.perf_counter() - t_gen
+    sup = wl["supports"]
+    nrow, nchan, npol = wl["uvw_m"].shape[0], cfg.n_chan, cfg.n_pol
+    g = Gridder(cfg.grid_n, wl["cell_rad"], cfg.n_wplanes, cfg.oversampling, int(sup.max()), npol, device=str(dev))
+    g.set_host_slices(args.host_slices)
+    g.allocate(sup, work_bytes=g.workspace_bytes(nrow, nchan, host=want_e2e))
+    t0 = time.perf_counter()
+    g.build_wkernels(wl["w_max"])
+    torch.cuda.synchronize(dev)
+    t_bank = time.perf_counter() - t0
+    g.set_compression(not args.no_compress)
+    if args.gather_min_support is not None:
+        g.set_gather_min_support(args.gather_min_support)
+
+    vis_f = np.ascontiguousarray(wl["vis"]).view(np.float32).reshape(nrow, nchan, npol, 2)
+    host = dict(uvw=wl["uvw_m"], bl=wl["baseline"], vis=vis_f, wt=wl["weights"])
+    if want_e2e:
+        host = {k: torch.from_numpy(np.ascontiguousarray(v)).pin_memory() for k, v in host.items()}
+        d = {k: v.to(dev, non_blocking=True) for k, v in host.items()}
+    else:
+        d = {k: torch.from_numpy(v).to(dev) for k, v in host.items()}
+    freqs = wl["freqs_hz"]
+    h2d_bytes = sum(int(v.numel() * v.element_size()) if hasattr(v, "numel") else v.nbytes for v in host.values()) + freqs.nbytes
+
+    def step():
+        g.grid_visibilities(d["uvw"], d["bl"], freqs, d["vis"], d["wt"])
+
+    def barrier():
+        ranks.barrier()
+        torch.cuda.synchronize(dev)
+
+    # one counted pass from a zero grid: statistics of ONE step (also the first warm-up)
+    g.reset()
+    g.set_commit_counting(True)
+    step()
+    gridded, dropped, updates = g.stats()
+    commits = g.commits()
+    compressed = g.compressed()
+    g.set_commit_counting(False)
+    touched = g.touched_pixels()
+    launches_per_step = g.last_launches()
+    for _ in range(max(0, warmup - 1)):
+        step()
+
+    sampler = ClockSampler(ranks.local).start() if (rank == 0 and sample_clocks) else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(steps):
+        step()
+    e1.record()
+    barrier()
+    ms_total = ranks.max_over_ranks(e0.elapsed_time(e1))
+    clocks = sampler.stop() if sampler else None
+    split = [g.timing(k) for k in range(min(steps, 64))]
+    ingest_ms = float(np.mean([s[0] for s in split]))
+    gridder_ms = float(np.mean([s[1] for s in split]))
+    ms_step = ms_total / steps
+
+    # end to end: host buffers through ig_grid_host, H2D copies and the D2H read of the step's result inside
+    e2e = None
+    if want_e2e:
+        def e2e_step():
+            g.grid_visibilities_host(host["uvw"], host["bl"], freqs, host["vis"], host["wt"])
+            return g.stats()                    # D2H read of the step's result (eq 4.17 counters), synchronises
+        e2e_step()
+        n_e2e = max(1, steps)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            e2e_step()
+        torch.cuda.synchronize(dev)
+        dt = ranks.max_over_ranks(time.perf_counter() - t0) / n_e2e
+        e2e = {"value": world * updates / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d_bytes), "d2h_bytes_per_step": 56,
+               "ms_per_step": dt * 1e3, "steps": n_e2e, "host_slices": args.host_slices,
+               "how": "ig_grid_host from pinned host buffers, slice k+1 copied while slice k is gridded, then ig_get_stats",
+               "result_residence": "by design the step's result, the uv-grid (%.2f GB), stays in HBM for further ig_grid calls and "
+                                   "ig_finalize (PAPER.md:1011: chunks are fed one after another); only the eq 4.17 counters "
+                                   "(56 B) are read back per step" % (g.grid.numel() * 4 / 1e9)}
+
+    roof = roofline_of(config, args.support_law, cfg, sup, nrow, nchan, npol, updates, commits, touched, gridder_ms,
+                       fp32_peak, commit_rate_l2)
+    hbm_peak, _ = peaks()
+    stride = 48 if npol == 4 else 32
+    ingest_bytes = nrow * nchan * (8 * npol + 4 * npol + stride) + nrow * (24 + 4 + 6 * 36)
+    res = {
+        "workload": WORKLOADS[config - 1], "ms_per_step": ms_step, "ingest_ms": ingest_ms, "gridder_ms": gridder_ms,
+        "updates_per_s": world * updates / (ms_step * 1e-3), "visibilities_per_s": world * gridded / (ms_step * 1e-3),
+        "gridder_updates_per_s": updates / (gridder_ms * 1e-3),
+        "records_gridded": gridded, "records_dropped": dropped, "updates_per_step": updates,
+        "records_compressed": compressed, "launches_per_step": launches_per_step, "steps": steps, "warmup": warmup,
+        "roofline": roof,
+        "ingest": {"bound": "hbm", "algorithmic_bytes": int(ingest_bytes), "achieved_gbs": ingest_bytes / (ingest_ms * 1e-3) / 1e9,
+                   "frac": ingest_bytes / (ingest_ms * 1e-3) / 1e9 / hbm_peak,
+                   "bytes_model": "per record vis 8 n_pol + weights 4 n_pol read, record written; per row uvw + permutation + 6 sort passes x 36 B"},
+        "clocks": clocks, "setup": {"generate_s": t_gen, "build_wkernels_s": t_bank},
+        "cfg": {"grid_n": cfg.grid_n, "n_pol": npol, "n_chan": nchan, "rows": int(nrow), "records": int(nrow) * nchan,
+                "w_planes": cfg.n_wplanes, "support": [int(sup.min()), int(sup.max())], "oversampling": cfg.oversampling},
+        "h2d_gb": h2d_bytes / 1e9, "e2e": e2e,
+    }
+    g.close()
+    del g, d, host, wl, vis_f
+    gc.collect()
+    torch.cuda.empty_cache()
+    return res
+
+
 def run_ours(args):
     import torch
     from paper_1403_4209_b200 import build as igbuild
     from paper_1403_4209_b200.binding import Gridder
-
     from paper_1403_4209_b200.dist import Ranks
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
@@ -199,137 +382,59 @@ def run_ours(args):
         igbuild.build()
     ranks.barrier()
 
-    def barrier():
-        ranks.barrier()
-        torch.cuda.synchronize(dev)
+    # device ceilings measured live: FP32 FMA peak and the L2-resident pixel-commit rate (red.global.add.v4.f32 pairs)
+    probe = Gridder(256, 1e-4, 1, 8, 7, 4, device=str(dev))
+    fp32_peak = probe.measure_fp32_peak()
+    commit_rate_l2 = probe.measure_commit_rate(32 << 20, run_len=-8)
+    probe.close()
 
-    max_over_ranks = ranks.max_over_ranks
-
-    cfg = synth.CONFIGS[args.config - 1]
-    t_gen = time.perf_counter()
-    wl = synth.make_workload(cfg, args.support_law)       # replicas only: every rank grids the same workload
-    t_gen = time.perf_counter() - t_gen
-    sup = wl["supports"]
-    nrow, nchan, npol = wl["uvw_m"].shape[0], cfg.n_chan, cfg.n_pol
-    g = Gridder(cfg.grid_n, wl["cell_rad"], cfg.n_wplanes, cfg.oversampling, int(sup.max()), npol, device=str(dev))
-    g.allocate(sup, work_bytes=g.workspace_bytes(nrow, nchan, host=not args.no_e2e))
-    t0 = time.perf_counter()
-    g.build_wkernels(wl["w_max"])
-    torch.cuda.synchronize(dev)
-    t_bank = time.perf_counter() - t0
-    fp32_peak = g.measure_fp32_peak()
-    g.set_compression(not args.no_compress)
-    g.set_host_slices(args.host_slices)
-
-    pin = (lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()) if not args.no_e2e else None
-    vis_f = np.ascontiguousarray(wl["vis"]).view(np.float32).reshape(nrow, nchan, npol, 2)
-    host = dict(uvw=wl["uvw_m"], bl=wl["baseline"], vis=vis_f, wt=wl["weights"])
-    if pin:
-        host = {k: pin(v) for k, v in host.items()}
-        d = {k: v.to(dev, non_blocking=True) for k, v in host.items()}
-    else:
-        d = {k: torch.from_numpy(v).to(dev) for k, v in host.items()}
-    freqs = wl["freqs_hz"]
-    h2d_bytes = sum(int(v.numel() * v.element_size()) if hasattr(v, "numel") else v.nbytes for v in host.values()) + freqs.nbytes
-
-    def step():
-        g.grid_visibilities(d["uvw"], d["bl"], freqs, d["vis"], d["wt"])
-
-    # one counted pass from a zero grid: statistics of ONE step (also the first warm-up)
-    g.reset()
-    g.set_commit_counting(True)
-    step()
-    gridded, dropped, updates = g.stats()
-    commits = g.commits()
-    compressed = g.compressed()
-    g.set_commit_counting(False)
-    touched = g.touched_pixels()
-    launches_per_step = g.last_launches()
-    for _ in range(max(0, args.warmup - 1)):
-        step()
-
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record()
-    for _ in range(args.steps):
-        step()
-    e1.record()
-    barrier()
-    ms_total = max_over_ranks(e0.elapsed_time(e1))
-    clocks = sampler.stop() if rank == 0 else None
-    split = [g.timing(k) for k in range(min(args.steps, 64))]
-    ingest_ms = float(np.mean([s[0] for s in split]))
-    gridder_ms = float(np.mean([s[1] for s in split]))
-    ms_step = ms_total / args.steps
-    value = world * updates / (ms_step * 1e-3)
-
-    # end to end: host buffers through ig_grid_host, H2D copies and the D2H read of the step's result inside
-    e2e = None
-    if not args.no_e2e:
-        def e2e_step():
-            g.grid_visibilities_host(host["uvw"], host["bl"], freqs, host["vis"], host["wt"])
-            return g.stats()                    # D2H read of the step's result (eq 4.17 counters), synchronises
-        e2e_step()
-        n_e2e = max(1, min(args.steps, 3))
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(n_e2e):
-            e2e_step()
-        torch.cuda.synchronize(dev)
-        dt = max_over_ranks(time.perf_counter() - t0) / n_e2e
-        e2e = {"value": world * updates / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d_bytes), "d2h_bytes_per_step": 56,
-               "ms_per_step": dt * 1e3, "steps": n_e2e, "host_slices": args.host_slices,
-               "how": "ig_grid_host from pinned host buffers, slice k+1 copied while slice k is gridded, then ig_get_stats"}
+    main = bench_config(args, args.config, dev, ranks, args.steps, args.warmup, not args.no_e2e, fp32_peak, commit_rate_l2, True)
+    per_config = {}
+    if not args.no_per_config:
+        for c in range(1, 6):
+            if c == args.config:
+                continue
+            r = bench_config(args, c, dev, ranks, max(3, min(args.steps, 10)), max(3, min(args.warmup, 5)), False, fp32_peak,
+                             commit_rate_l2, True)
+            per_config[WORKLOADS[c - 1]] = {k: r[k] for k in ("ms_per_step", "ingest_ms", "gridder_ms", "updates_per_s", "visibilities_per_s",
+                                                              "updates_per_step", "records_gridded", "steps", "warmup", "clocks")}
+            per_config[WORKLOADS[c - 1]]["roofline"] = {k: r["roofline"][k] for k in ("bound", "frac", "frac_alu", "frac_hbm_model", "t_flop_ms",
+                                                                                     "t_byte_ms", "commits", "commits_measured")}
+            per_config[WORKLOADS[c - 1]]["ingest_achieved_gbs"] = r["ingest"]["achieved_gbs"]
 
     if rank != 0:
         ranks.close()
         return
 
-    # ---- roofline of the dominant kernel (k_gridder), DESIGN.md "Roofline" -------------------------
-    hbm_peak, peak_src = peaks()
-    stride = 48 if npol == 4 else 32
-    n_chunks = ((nrow + 127) // 128) * nchan
-    bank_bytes = int((sup.astype(np.int64) ** 2).sum()) * cfg.oversampling ** 2 * 8
-    alg_bytes = n_chunks * 128 * stride + bank_bytes + commits * 8 * npol + touched * 8 * npol * 2
-    t_byte = alg_bytes / (hbm_peak * 1e9)
-    flops = 8.0 * updates
-    t_flop = flops / (fp32_peak * 1e12)
-    gs = gridder_ms * 1e-3
-    if t_byte >= t_flop:
-        roof = {"bound": "hbm", "achieved": alg_bytes / gs / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                "frac": t_byte / gs, "traffic": ncu_traffic(args.config), "peak_source": peak_src}
-    else:
-        roof = {"bound": "alu", "achieved": flops / gs / 1e12, "peak": fp32_peak, "unit": "TFLOP/s",
-                "frac": t_flop / gs, "traffic": ncu_traffic(args.config), "peak_source": "measured live: ig_measure_fp32_peak (FFMA loop)"}
-    roof.update({"kernel": "k_gridder", "kernel_ms": gridder_ms, "t_flop_ms": t_flop * 1e3, "t_byte_ms": t_byte * 1e3,
-                 "algorithmic_bytes": int(alg_bytes), "flops": flops, "fp32_peak_tflops": fp32_peak, "hbm_peak_gbs": hbm_peak,
-                 "commits": commits, "touched_pixels": touched})
-
+    cfg = synth.CONFIGS[args.config - 1]
     cpu = None
     if not args.no_cpu and world == 1:
         c = cpu_oracle_sample(cfg, args.support_law, args.cpu_seconds)
+        c1 = cpu_oracle_sample(cfg, args.support_law, 5.0, n_threads=1)
         cpu = {"value": c["value"], "unit": UNIT, "cores": c["cores"], "kind": "oracle", "sample": c["sample"],
-               "seconds": c["seconds"]}
+               "seconds": c["seconds"], "single_thread": {"value": c1["value"], "seconds": c1["seconds"], "sample": c1["sample"]}}
+        if args.cpu_full:
+            cpu["full_size"] = {}
+            for k in (0, 1, 2):
+                f = cpu_oracle_sample(synth.CONFIGS[k], args.support_law, 0.0, full=True)
+                cpu["full_size"][WORKLOADS[k]] = {"value": f["value"], "seconds": f["seconds"], "records": f["records"], "cores": f["cores"]}
 
+    cc = main["cfg"]
     out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "metric": METRIC, "value": main["updates_per_s"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
-        "config": {"workload": WORKLOADS[args.config - 1], "grid_n": cfg.grid_n, "n_pol": npol, "n_chan": nchan, "rows": int(nrow),
-                   "records": int(nrow) * nchan, "w_planes": cfg.n_wplanes, "support": [int(sup.min()), int(sup.max())],
-                   "support_law": args.support_law, "oversampling": cfg.oversampling, "parallelism": f"replicas x{world}",
-                   "l2": "inputs (%.1f GB) larger than L2; no flush needed" % (h2d_bytes / 1e9)},
-        "visibilities_per_s": world * gridded / (ms_step * 1e-3),
-        "records_gridded": gridded, "records_dropped": dropped, "updates_per_step": updates,
-        "compression": {"enabled": not args.no_compress, "records_compressed": compressed,
+        "config": {"workload": main["workload"], **cc, "support_law": args.support_law, "parallelism": f"replicas x{world}",
+                   "l2": "inputs (%.1f GB) larger than L2; no flush needed" % main["h2d_gb"]},
+        "visibilities_per_s": main["visibilities_per_s"],
+        "records_gridded": main["records_gridded"], "records_dropped": main["records_dropped"], "updates_per_step": main["updates_per_step"],
+        "compression": {"enabled": not args.no_compress, "records_compressed": main["records_compressed"],
                         "note": "value counts every gridded record (thesis total rate, PAPER.md:1767); "
                                 "real rate = value * (1 - records_compressed / records_gridded)"},
-        "ingest_ms": ingest_ms, "gridder_ms": gridder_ms, "gridder_updates_per_s": updates / gs,
-        "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
-        "clocks": clocks, "setup": {"generate_s": t_gen, "build_wkernels_s": t_bank},
+        "ingest_ms": main["ingest_ms"], "gridder_ms": main["gridder_ms"], "gridder_updates_per_s": main["gridder_updates_per_s"],
+        "roofline": main["roofline"], "ingest": main["ingest"], "cpu_baseline": cpu, "e2e": main["e2e"],
+        "gpu_launches": main["launches_per_step"] * args.steps,
+        "clocks": main["clocks"], "setup": main["setup"], "per_config": per_config,
         "context": "thesis GTX 680: ~50 G updates/s real rate, Romein 93 G (PAPER.md:742,:1986) - other hardware, not a target",
     }
     print(json.dumps(out))

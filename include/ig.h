@@ -42,14 +42,15 @@ typedef enum {
 } ig_status;
 
 #define IG_C_M_S 299792458.0 /* speed of light used for metres -> wavelengths */
-#define IG_MAX_SUPPORT 255   /* record headers carry the support in 8 bits */
+#define IG_MAX_SUPPORT 511   /* largest support the thesis sweeps (:1785-1789); record headers carry it in 9 bits */
 
 /* Create a context. No device work.
  *   grid_n        grid side N, even, 16..32768
  *   cell_rad      image pixel size in radians; uv cell du = 1/(N*cell_rad) wavelengths
  *   n_wplanes     P >= 1 w-planes spaced in sqrt(w) (:633,:1068); 1 = plain gridding
  *   oversampling  beta in 1..16 (eq 2.11 :548)
- *   max_support   largest kernel support, odd, 3..IG_MAX_SUPPORT
+ *   max_support   largest kernel support, odd, 3..IG_MAX_SUPPORT (the thesis's heavy configuration needs
+ *                 349, :1924); a valid odd support above IG_MAX_SUPPORT returns IG_EUNSUPPORTED
  *   n_pol         1, 2 or 4 polarisations (:1025,:1377)                           */
 ig_status ig_create(ig_ctx** out, int grid_n, double cell_rad, int n_wplanes, int oversampling,
                     int max_support, int n_pol);
@@ -108,17 +109,21 @@ ig_status ig_debug_get_wkernels(ig_ctx* ctx, float* bank_host, size_t bank_bytes
  *      visibility (eq 4.16);  A3 records whose footprint leaves the grid or whose weights
  *      are all zero are dropped (:1278,:1315), the stream is cut into work items;
  *   C  the gridder.
- *   uvw_m        dev f64 [nrow][3], metres
+ *   uvw_m        dev f64 [nrow][3], metres; a row with a NaN or infinite coordinate is dropped (reading 20)
  *   baseline_id  dev i32 [nrow], any non-negative ids; rows in any order
  *   freqs_hz     HOST f64 [nchan]
  *   vis          dev f32 [nrow][nchan][n_pol][2]
  *   weights      dev f32 [nrow][nchan][n_pol]; weight 0 = flagged (:1286)
+ * All arrays dense (no strides) and naturally aligned; with n_pol = 4 vis and weights are read as 16-byte
+ * vectors and must be 16-byte aligned (IG_EINVAL otherwise).
  * Asynchronous; inputs must stay valid until the stream reaches the end of the call. */
 ig_status ig_grid(ig_ctx* ctx, const double* uvw_m, const int* baseline_id, long long nrow,
                   const double* freqs_hz, int nchan, const float* vis, const float* weights);
 
-/* Same, with HOST inputs: copies them to staging areas inside work_dev (which must be
- * ig_workspace_bytes() + ig_host_staging_bytes() large) and grids. The end-to-end leg. */
+/* Same, with HOST inputs: copies them to staging areas inside work_dev and grids. The end-to-end leg.
+ * work_dev must hold ig_workspace_bytes(ctx, nrow, nchan) + ig_host_staging_bytes(ctx, nrow, nchan) (an upper
+ * bound: a sliced batch needs the workspace of one slice plus two slice-sized staging areas, which is what
+ * ig_host_staging_bytes counts for the ig_set_host_slices value in force when it is called). */
 size_t ig_host_staging_bytes(const ig_ctx* ctx, long long nrow, int nchan);
 /* ig_grid_host cuts the rows into n slices (default 8; 1 = no slicing; batches under 65 536 rows are never
  * sliced) and copies slice k+1 on a second stream while slice k is gridded. The copies overlap the kernels only
@@ -134,6 +139,17 @@ ig_status ig_grid_host(ig_ctx* ctx, const double* uvw_m, const int* baseline_id,
  *   normaliser_host  HOST f64 [n_pol], receives N_p; may be NULL
  * Uses work_dev (ig_finalize_workspace_bytes()). Synchronises. */
 ig_status ig_finalize(ig_ctx* ctx, float* image_dev, double* normaliser_host);
+
+/* Step C runs two work distributions: records with support < s keep Romein's moving window
+ * (registers follow a track, atomics when a pixel leaves the window, :710-742); records with support >= s go to
+ * the fixed-tile gather gridder (a warp owns an 8 x 16 pixel tile in registers, records binned by tile, no atomics
+ * in the loop). Default 17. s = 1: everything through the gather gridder; s > IG_MAX_SUPPORT: nothing. Same grid
+ * up to fp32 summation order. Per-channel grids always use the moving window. */
+ig_status ig_set_gather_min_support(ig_ctx* ctx, int s);
+
+/* Ordering (A2): rows are sorted by (uv tile in Morton order, baseline, time). shift = log2 of the tile side in
+ * cells, 5..15; 0 = automatic (N/8 cells, at least 128). A tuning knob for experiments; the grid does not depend on it. */
+ig_status ig_set_sort_tile_shift(ig_ctx* ctx, int shift);
 
 /* One grid per channel (the thesis's default mode, :1011, :1120; reading 16): with the switch on, grid_dev holds nchan
  * grids back to back (each ig_grid_bytes(), same layout), channel c of every ig_grid call goes to grid c with its own
@@ -157,8 +173,9 @@ ig_status ig_get_commits(ig_ctx* ctx, long long* n_commits);
  * the ig_grid calls whose commits are to be counted (bench.py's counted pass). */
 ig_status ig_set_commit_counting(ig_ctx* ctx, int on);
 /* Measured FP32 FMA peak of the device in TFLOP/s (register-only FFMA loop on every SM, timed
- * with CUDA events on `cuda_stream`): the ALU denominator of the gridding roofline. */
-ig_status ig_measure_fp32_peak(void* cuda_stream, double* tflops);
+ * with CUDA events on `cuda_stream`): the ALU denominator of the gridding roofline.
+ * sink_dev: dev, 4 bytes owned by the caller (written only by a branch that is never taken). */
+ig_status ig_measure_fp32_peak(void* cuda_stream, void* sink_dev, double* tflops);
 /* Measured rate of the gridder's commit (one 32-byte 4-pol pixel = 2 x red.global.add.v4.f32) at
  * pseudo-random places of buf_dev (dev, `bytes` long, contents are added to), in 1e9 pixel commits/s.
  * run_len = consecutive pixels committed by neighbouring lanes (1..32). The atomic ceiling of the

@@ -49,7 +49,8 @@ void orc_constants(int grid_n, double cell_rad, int beta, int n_wplanes, double 
  *   X,Y      centre cell (pixel N/2 is u=v=0, :1319-1321)
  *   off_u/v  sub-cell offset in oversampled samples, in (-beta/2, beta/2]
  *   plane    w-plane, nearest in sqrt(w)
- *   flags    bit0 = conjugated (w<0), bit1 = whole footprint on the grid */
+ *   flags    bit0 = conjugated (w<0), bit1 = whole footprint on the grid
+ * A record with a non-finite coordinate (NaN or inf in u, v or w) is off the grid. */
 void orc_index(int64_t nrow, int nchan, const double *uvw_m, const double *freqs_hz,
                int grid_n, double cell_rad, int beta, int n_wplanes, double w_max,
                const int32_t *support, int32_t *X, int32_t *Y, int32_t *off_u,
@@ -65,6 +66,13 @@ void orc_index(int64_t nrow, int nchan, const double *uvw_m, const double *freqs
             double nu = freqs_hz[c];
             double fu = (um * nu) * ku; /* (u/lambda) * beta/du, eq 1.7 + eq 2.11 */
             double fv = (vm * nu) * ku;
+            int64_t k = r * nchan + c;
+            if (!(isfinite(fu) && isfinite(fv) && isfinite(wm * nu))) {
+                /* a non-finite coordinate has no cell (reading 20): the record is dropped like one
+                 * whose footprint leaves the grid (:1278); its tuple is all zero apart from the conj bit */
+                X[k] = 0; Y[k] = 0; off_u[k] = 0; off_v[k] = 0; plane[k] = 0; flags[k] = conj;
+                continue;
+            }
             int64_t U = (int64_t)ceil(fu - 0.5); /* nearest sample, ties to -inf */
             int64_t V = (int64_t)ceil(fv - 0.5);
             int64_t x = floordiv64(U + half_up - 1, beta); /* eq 4.2: -du/2 < delta <= du/2 */
@@ -78,7 +86,6 @@ void orc_index(int64_t nrow, int nchan, const double *uvw_m, const double *freqs
             int64_t h = (support[p] - 1) / 2;
             int64_t Xc = x + grid_n / 2, Yc = y + grid_n / 2;
             int on = (Xc - h >= 0) && (Xc + h <= grid_n - 1) && (Yc - h >= 0) && (Yc + h <= grid_n - 1);
-            int64_t k = r * nchan + c;
             /* clamp far-off cells so they fit int32; they are off-grid anyway */
             if (Xc < -(1 << 30)) Xc = -(1 << 30);
             if (Xc > (1 << 30)) Xc = (1 << 30);
@@ -163,6 +170,15 @@ void orc_grid(int64_t nrow, int nchan, int npol, const float *vis /*[nrow][nchan
     }
     for (int q = 0; q < npol; ++q) norm[q] += nsum[q];
     stats[0] += gridded; stats[1] += dropped; stats[2] += updates;
+}
+
+/* measurement infrastructure only: thread count of the next orc_grid calls (0 = the OpenMP default) */
+void orc_set_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
 }
 
 int orc_threads(void) {

@@ -154,18 +154,20 @@ def auto_supports(n_wplanes, w_max, du, beta, max_support, threshold=1e-3):
     return out
 
 
-def build_bank(supports, w_max, du, beta, max_support):
+def build_bank(supports, w_max, du, beta, max_support, planes=None):
     """Returns (bank complex128 flat, bank_off int64[P]).
     K[p][ov][ou][ty][tx] = C_p[ty*beta - off_v][tx*beta - off_u], ty,tx in [-h,h],
-    ov = off_v + ceil(beta/2) - 1 (eq 4.1 :1078 with reading 1; layout :1100-1108)."""
+    ov = off_v + ceil(beta/2) - 1 (eq 4.1 :1078 with reading 1; layout :1100-1108).
+    planes: optional subset of plane indices to compute; the other planes of the bank stay zero
+    (for checks of a window of a large grid that only a few planes reach)."""
     supports = np.asarray(supports, dtype=np.int64)
     P = supports.size
     n = inner_samples(int(max_support))
     shift = (beta + 1) // 2 - 1
     off = np.zeros(P, dtype=np.int64)
     off[1:] = np.cumsum(supports[:-1] ** 2 * beta * beta)
-    bank = np.empty(int((supports ** 2).sum() * beta * beta), dtype=np.complex128)
-    for p in range(P):
+    bank = np.zeros(int((supports ** 2).sum() * beta * beta), dtype=np.complex128)
+    for p in (range(P) if planes is None else sorted(set(int(x) for x in planes))):
         S = int(supports[p]); h = (S - 1) // 2
         qmax = h * beta + beta          # covers every ty*beta - off
         C = oversampled_kernel(p, P, w_max, du, beta, n, -qmax, qmax)
@@ -237,6 +239,11 @@ def grid_records(idx, vis, weights, grid_n, beta, supports, bank, bank_off, grid
 
 def threads() -> int:
     return int(_lib().orc_threads())
+
+
+def set_threads(n: int) -> None:
+    """Thread count of the following grid_records calls (timing the single-thread rate)."""
+    _lib().orc_set_threads(ctypes.c_int(int(n)))
 
 
 # ----------------------------------------------------------------------------

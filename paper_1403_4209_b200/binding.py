@@ -43,7 +43,9 @@ SIGNATURES = {
     "ig_set_compression": (_i, [_vp, _i]),
     "ig_get_compressed": (_i, [_vp, C.POINTER(_ll)]),
     "ig_set_commit_counting": (_i, [_vp, _i]),
-    "ig_measure_fp32_peak": (_i, [_vp, C.POINTER(_d)]),
+    "ig_measure_fp32_peak": (_i, [_vp, _vp, C.POINTER(_d)]),
+    "ig_set_sort_tile_shift": (_i, [_vp, _i]),
+    "ig_set_gather_min_support": (_i, [_vp, _i]),
     "ig_measure_commit_rate": (_i, [_vp, _vp, _sz, _i, C.POINTER(_d)]),
     "ig_get_timing": (_i, [_vp, _i, C.POINTER(C.c_float), C.POINTER(C.c_float)]),
     "ig_reset_accumulators": (_i, [_vp]),
@@ -174,7 +176,7 @@ class Gridder:
     def workspace_bytes(self, nrow, nchan, host=False):
         n = self.lib.ig_workspace_bytes(self.ctx, nrow, nchan)
         if host:
-            n += 256 + self.lib.ig_host_staging_bytes(self.ctx, nrow, nchan)
+            n += self.lib.ig_host_staging_bytes(self.ctx, nrow, nchan)
         return n
 
     # -- the calls of include/ig.h ----------------------------------------------------
@@ -196,11 +198,34 @@ class Gridder:
         self._check(self.lib.ig_debug_get_wkernels(self.ctx, _np_ptr(out), out.nbytes), "ig_debug_get_wkernels")
         return out
 
+    def _check_inputs(self, uvw_m, baseline_id, vis, weights, nrow, nchan, on_device):
+        """The C ABI takes bare pointers: dtype, density, element count and residence are checked here."""
+        t = self.torch
+        want = (("uvw_m", uvw_m, ("float64",), nrow * 3), ("baseline_id", baseline_id, ("int32",), nrow),
+                ("vis", vis, ("float32", "complex64"), None), ("weights", weights, ("float32",), nrow * nchan * self.n_pol))
+        for name, a, dtypes, numel in want:
+            is_t = isinstance(a, t.Tensor)
+            dt = str(a.dtype).replace("torch.", "")
+            if dt not in dtypes:
+                raise IgError(f"{name}: dtype {dt}, expected {dtypes}")
+            if numel is None:
+                numel = nrow * nchan * self.n_pol * (1 if dt == "complex64" else 2)
+            n = a.numel() if is_t else a.size
+            if n != numel:
+                raise IgError(f"{name}: {n} elements, expected {numel}")
+            if not (a.is_contiguous() if is_t else a.flags["C_CONTIGUOUS"]):
+                raise IgError(f"{name}: not contiguous")
+            if on_device and not (is_t and a.is_cuda and a.device == self.device):
+                raise IgError(f"{name}: must be a tensor on {self.device}")
+            if not on_device and is_t and a.is_cuda:
+                raise IgError(f"{name}: must be host memory")
+
     def grid_visibilities(self, uvw_m, baseline_id, freqs_hz, vis, weights):
         """Device tensors: uvw_m f64 [nrow,3], baseline_id i32 [nrow], vis c64/f32 [nrow,nchan,npol(,2)],
         weights f32 [nrow,nchan,npol]; freqs_hz: host numpy f64."""
         freqs = np.ascontiguousarray(freqs_hz, dtype=np.float64)
         nrow, nchan = int(uvw_m.shape[0]), int(freqs.size)
+        self._check_inputs(uvw_m, baseline_id, vis, weights, nrow, nchan, on_device=True)
         self.ensure_work(self.workspace_bytes(nrow, nchan))
         self._check(self.lib.ig_grid(self.ctx, _vp(uvw_m.data_ptr()), _vp(baseline_id.data_ptr()), nrow,
                                      _np_ptr(freqs), nchan, _vp(vis.data_ptr()), _vp(weights.data_ptr())), "ig_grid")
@@ -209,6 +234,7 @@ class Gridder:
         """Same with HOST buffers (numpy arrays or pinned CPU torch tensors): the end-to-end call."""
         freqs = np.ascontiguousarray(freqs_hz, dtype=np.float64)
         nrow, nchan = int(uvw_m.shape[0]), int(freqs.size)
+        self._check_inputs(uvw_m, baseline_id, vis, weights, nrow, nchan, on_device=False)
         self.ensure_work(self.workspace_bytes(nrow, nchan, host=True))
         ptr = lambda a: _vp(a.data_ptr()) if hasattr(a, "data_ptr") else _np_ptr(a)
         self._check(self.lib.ig_grid_host(self.ctx, ptr(uvw_m), ptr(baseline_id), nrow, _np_ptr(freqs), nchan,
@@ -230,6 +256,12 @@ class Gridder:
     def set_host_slices(self, n: int):
         self._check(self.lib.ig_set_host_slices(self.ctx, int(n)), "ig_set_host_slices")
 
+    def set_gather_min_support(self, s: int):
+        self._check(self.lib.ig_set_gather_min_support(self.ctx, int(s)), "ig_set_gather_min_support")
+
+    def set_sort_tile_shift(self, shift: int):
+        self._check(self.lib.ig_set_sort_tile_shift(self.ctx, int(shift)), "ig_set_sort_tile_shift")
+
     def set_compression(self, on: bool):
         self._check(self.lib.ig_set_compression(self.ctx, int(bool(on))), "ig_set_compression")
 
@@ -248,7 +280,8 @@ class Gridder:
 
     def measure_fp32_peak(self) -> float:
         v = _d()
-        self._check(self.lib.ig_measure_fp32_peak(self._stream_ptr(), C.byref(v)), "ig_measure_fp32_peak")
+        sink = self.torch.zeros(1, dtype=self.torch.float32, device=self.device)
+        self._check(self.lib.ig_measure_fp32_peak(self._stream_ptr(), _vp(sink.data_ptr()), C.byref(v)), "ig_measure_fp32_peak")
         return v.value
 
     def measure_commit_rate(self, nbytes, run_len=8) -> float:
@@ -288,6 +321,16 @@ class Gridder:
         if self.n_pol == 4:
             n = self.grid_n
             g = g.view(2, n, n, 2, 2).permute(1, 2, 0, 3, 4).reshape(n, n, 4, 2)
+        return g.contiguous().cpu().numpy().view(np.complex64)[..., 0]
+
+    def grid_window_complex(self, x0, y0, w, h) -> np.ndarray:
+        """Pixels [y0, y0+h) x [x0, x0+w) of the grid as complex64 numpy [h][w][npol] (synchronises)."""
+        self.torch.cuda.synchronize(self.device)
+        n = self.grid_n
+        if self.n_pol == 4:
+            g = self.grid.view(2, n, n, 2, 2)[:, y0:y0 + h, x0:x0 + w].permute(1, 2, 0, 3, 4).reshape(h, w, 4, 2)
+        else:
+            g = self.grid[y0:y0 + h, x0:x0 + w]
         return g.contiguous().cpu().numpy().view(np.complex64)[..., 0]
 
     def touched_pixels(self) -> int:

@@ -25,7 +25,7 @@ bool table_ok(const ig_ctx* c, const int* t) {
         if (t[p] < 1 || t[p] > c->max_support || (t[p] & 1) == 0) return false;
     return true;
 }
-struct GridLayout { size_t freqs, perm, sort, smax, records, total; long long nrb, n_chunks; };
+struct GridLayout { size_t freqs, perm, sort, smax, gcount, tile_count, tile_off, tile_cur, plan_hdr, items, records, entries, total; long long nrb, n_chunks; };
 GridLayout grid_layout(const ig_ctx* c, long long nrow, int nchan) {
     GridLayout L{};
     L.nrb = (nrow + IG_CH - 1) / IG_CH;
@@ -35,7 +35,16 @@ GridLayout grid_layout(const ig_ctx* c, long long nrow, int nchan) {
     L.perm = o; o += ig_align((size_t)nrow * 4);
     L.sort = o; o += ig_align(ig_sort_scratch_bytes(nrow));
     L.smax = o; o += ig_align((size_t)L.n_chunks * 4);
-    L.records = o; o += ig_align((size_t)L.n_chunks * IG_CH * ig_rec_stride(c->prm.npol));
+    L.gcount = o; o += ig_align((size_t)L.n_chunks * 4);          // directly after smax (cleared together)
+    const size_t nt = ig_gather_tiles(c);
+    L.tile_count = o; o += ig_align(nt * 4);
+    L.tile_off = o; o += ig_align(nt * 4);
+    L.tile_cur = o; o += ig_align(nt * 4);
+    L.plan_hdr = o; o += 256;
+    L.items = o; o += ig_align(ig_gather_max_items(c, L.n_chunks) * 16);
+    const size_t rec_bytes = ig_align((size_t)L.n_chunks * IG_CH * ig_rec_stride(c->prm.npol));
+    L.records = o; o += rec_bytes;
+    L.entries = o; o += ig_align((size_t)L.n_chunks * IG_CH * (16 + 16 * c->prm.npol));   // gather entries: at most every record
     L.total = o;
     return L;
 }
@@ -71,7 +80,8 @@ ig_status ig_create(ig_ctx** out, int grid_n, double cell_rad, int n_wplanes, in
     if (!(cell_rad > 0.0) || !isfinite(cell_rad)) return IG_EINVAL;
     if (n_wplanes < 1 || n_wplanes > (1 << 20)) return IG_EINVAL;
     if (oversampling < 1 || oversampling > 16) return IG_EINVAL;
-    if (max_support < 3 || max_support > IG_MAX_SUPPORT || (max_support & 1) == 0 || max_support > grid_n) return IG_EINVAL;
+    if (max_support < 3 || (max_support & 1) == 0 || max_support > grid_n) return IG_EINVAL;
+    if (max_support > IG_MAX_SUPPORT) return IG_EUNSUPPORTED;   // record headers carry c, d, S in 9 bits each
     if (n_pol != 1 && n_pol != 2 && n_pol != 4) return IG_EINVAL;
     ig_ctx* c = new (std::nothrow) ig_ctx();
     if (!c) return IG_ENOMEM;
@@ -108,11 +118,15 @@ size_t ig_bank_bytes(const ig_ctx* c, const int* table) {
     return bank_head_bytes(c) + ig_align(bank_elems_of(c, table) * 8);
 }
 size_t ig_finalize_workspace_bytes(const ig_ctx* c) { return c ? ig_finalize_scratch_bytes(c) : 0; }
+static long long host_slice_rows(const ig_ctx* c, long long nrow);
+static size_t host_stage_bytes(const ig_ctx* c, long long rows, int nchan);
 size_t ig_host_staging_bytes(const ig_ctx* c, long long nrow, int nchan) {
     if (!c || nrow < 0 || nchan < 1) return 0;
-    // room for an unsliced copy of everything: an upper bound for any slice count (two slice buffers need less)
-    size_t rec = (size_t)nrow * nchan * c->prm.npol;
-    return ig_align((size_t)nrow * 24) + ig_align((size_t)nrow * 4) + ig_align(rec * 8) + ig_align(rec * 4) + 4096;
+    // what ig_grid_host carves after the first ig_workspace_bytes(): one staging area for an unsliced batch, two
+    // (double buffering) when the rows are cut into slices; sized for the current ig_set_host_slices() value
+    const long long srows = host_slice_rows(c, nrow);
+    const size_t pad = ig_align(ig_workspace_bytes(c, srows, nchan)) - ig_workspace_bytes(c, srows, nchan);
+    return pad + (srows < nrow ? 2 : 1) * host_stage_bytes(c, srows, nchan);
 }
 
 ig_status ig_bind(ig_ctx* c, void* grid_dev, size_t grid_bytes, void* work_dev, size_t work_bytes, void* bank_dev,
@@ -217,6 +231,8 @@ ig_status ig_grid(ig_ctx* c, const double* uvw, const int* baseline_id, long lon
     c->launches = 0;
     if (nrow == 0) return IG_OK;
     if (!uvw || !baseline_id || !vis || !wt) return fail(c, IG_EINVAL, "null input");
+    if (((uintptr_t)uvw & 7) || ((uintptr_t)baseline_id & 3) || (((uintptr_t)vis | (uintptr_t)wt) & (c->prm.npol == 4 ? 15 : 3)))
+        return fail(c, IG_EINVAL, "misaligned input (n_pol = 4: vis and weights must be 16-byte aligned)");
     GridLayout L = grid_layout(c, nrow, nchan);
     if (L.total > c->work_bytes) return fail(c, IG_ENOMEM, "work buffer smaller than ig_workspace_bytes()");
     double* d_freqs = (double*)(c->work + L.freqs);
@@ -232,13 +248,26 @@ ig_status ig_grid(ig_ctx* c, const double* uvw, const int* baseline_id, long lon
     int n = ig_launch_sort_rows(c, uvw, baseline_id, nrow, fref, perm, c->work + L.sort, ig_sort_scratch_bytes(nrow));
     if (n < 0) return IG_ECUDA;
     c->launches += n;
-    n = ig_launch_index(c, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, smax);
+    uint32_t* gcount = (uint32_t*)(c->work + L.gcount);
+    uint32_t* tile_count = (uint32_t*)(c->work + L.tile_count);
+    // per-channel grids keep every record with the moving-window gridder (the tile plan is per grid)
+    const int gather_min = c->per_channel ? (IG_MAX_SUPPORT + 1) : c->gather_min;
+    n = ig_launch_index(c, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, smax, gcount, tile_count, gather_min);
     if (n < 0) return IG_ECUDA;
     c->launches += n;
     cudaEventRecord(ev[1], c->stream);
     n = ig_launch_gridder(c, records, smax, L.nrb, nchan);
     if (n < 0) return IG_ECUDA;
     c->launches += n;
+    bool any_gather = false;
+    for (int p = 0; p < c->prm.P; ++p) any_gather |= c->support[p] >= gather_min;
+    if (any_gather) {
+        n = ig_launch_gather(c, records, gcount, L.n_chunks, tile_count, (uint32_t*)(c->work + L.tile_off),
+                             (uint32_t*)(c->work + L.tile_cur), (uint4*)(c->work + L.items), (uint32_t*)(c->work + L.plan_hdr),
+                             c->work + L.entries);
+        if (n < 0) return IG_ECUDA;
+        c->launches += n;
+    }
     cudaEventRecord(ev[2], c->stream);
     c->n_timed += 1;
     return IG_OK;
@@ -250,8 +279,10 @@ ig_status ig_grid(ig_ctx* c, const double* uvw, const int* baseline_id, long lon
 static long long host_slice_rows(const ig_ctx* c, long long nrow) {
     int k = c->host_slices;
     if (nrow < (1 << 16)) k = 1;
+    if (k == 1) return nrow;                         // unsliced: ig_grid takes a partial last row block
     long long r = (nrow + k - 1) / k;
-    return (r + IG_CH - 1) / IG_CH * IG_CH;          // whole row blocks
+    r = (r + IG_CH - 1) / IG_CH * IG_CH;             // whole row blocks
+    return r < nrow ? r : nrow;
 }
 static size_t host_stage_bytes(const ig_ctx* c, long long rows, int nchan) {
     size_t rec = (size_t)rows * nchan * c->prm.npol;
@@ -272,10 +303,10 @@ ig_status ig_grid_host(ig_ctx* c, const double* uvw, const int* baseline_id, lon
     if (nrow == 0) return IG_OK;
     if (!uvw || !baseline_id || !vis || !wt) return fail(c, IG_EINVAL, "null input");
     const long long srows = host_slice_rows(c, nrow);
-    const size_t base = ig_align(grid_layout(c, srows, nchan).total);
+    const size_t base = ig_align(ig_workspace_bytes(c, srows, nchan));
     const size_t stage = host_stage_bytes(c, srows, nchan);
     const int nbuf = srows < nrow ? 2 : 1;
-    if (base + nbuf * stage > c->work_bytes) return fail(c, IG_ENOMEM, "work buffer smaller than ig_workspace_bytes() + ig_host_staging_bytes()");
+    if (base + nbuf * stage > c->work_bytes) return fail(c, IG_ENOMEM, "work buffer smaller than ig_workspace_bytes(slice rows) + ig_host_staging_bytes()");
     if (!c->copy_stream) {
         if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(c, IG_ECUDA, "cannot create the copy stream");
         for (auto& e : c->ev_copied) cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
@@ -310,6 +341,18 @@ ig_status ig_grid_host(ig_ctx* c, const double* uvw, const int* baseline_id, lon
         if (e != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_grid_host: ") + cudaGetErrorString(e));
     }
     c->launches = launches;
+    return IG_OK;
+}
+
+ig_status ig_set_gather_min_support(ig_ctx* c, int s) {
+    if (!c || s < 1) return IG_EINVAL;
+    c->gather_min = s;
+    return IG_OK;
+}
+
+ig_status ig_set_sort_tile_shift(ig_ctx* c, int shift) {
+    if (!c || (shift != 0 && (shift < 5 || shift > 15))) return IG_EINVAL;
+    c->tile_shift = shift;
     return IG_OK;
 }
 

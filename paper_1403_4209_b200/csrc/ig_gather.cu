@@ -1,0 +1,373 @@
+// ig_gather.cu - step C for LARGE supports: the fixed-tile ("gather") gridder and its plan (steps A3 + C).
+//
+//   grid[Y0+ty][X0+tx][pol] += a[pol] * K[p][ov][ou][ty][tx]      (eq 4.4a/b)
+//
+// Why a second work distribution. Romein's moving window (ig_gridder.cu) keeps a sum in a
+// register only while successive records of ONE track overlap; on long baselines with supports of 17..129 cells
+// the window moves by many cells per record, 40-45 % of all register sums end in an atomic (oracle/track_commits.py)
+// and the L2 atomic unit, not the FP32 pipe, sets the pace (config 5: 26 G pixel commits). Here the ownership is
+// turned round: a warp owns a FIXED 8 x 16 pixel tile of the grid in registers (4 pixels per lane, all
+// polarisations), and every record whose footprint crosses the tile - of any baseline, time or channel - is
+// accumulated into those registers; the tile is written once per work item. No atomics in the loop, contributions
+// of different tracks combine on chip, and the per-(record, pixel) work is a compare, an address, one read-only
+// load and the FMAs. The price is lanes outside the footprint (efficiency ~ S/(S+7) * S/(S+3)), so supports below
+// `gather_min_support` stay with the moving window, where tracks overlap well and the tile would be mostly idle.
+// The thesis had two kernels split at S = 31 for a similar reason (:1371-1379); shared memory is not used for the
+// sums (fp32 shared atomics are CAS loops, and a read-modify-write per tap is 4x the FP32 pipe time).
+//
+// Plan (the thesis's scan / compaction / plan steps, Alg 4.2-4.3 :1446-1508, rebuilt for this ownership):
+//   k_index            marks large-support records (IG_HDR_GATHER) and counts them per 32 x 32 "origin tile"
+//                      (the tile that holds the footprint's first pixel)
+//   k_gather_plan      one CTA: exclusive scan of the counts -> tile offsets; cuts every tile's list into items
+//                      of <= IG_GCH records
+//   k_gather_scatter   counting-sort scatter of the marked records into tile order (header rewritten relative
+//                      to the tile)
+//   k_gather           persistent CTAs; an item's records are staged once into shared memory by the TMA bulk-copy
+//                      engine; the CTA's warps take the 8 x 16 sub-tiles of the region the item can reach
+//                      (32 + Smax - 1 pixels on a side) from a shared counter; per sub-tile a ballot over the
+//                      staged headers finds the records that touch it.
+#include "ig_internal.h"
+
+#define IG_GT 32          // origin tile side in pixels
+#define IG_GT_SHIFT 5
+#define IG_GCH 256        // records per gather item
+#define IG_GW 8           // warps per gather CTA
+#define IG_GR 4           // pixel row groups per lane: sub-tile = 8 wide x 4*IG_GR tall
+#define IG_GCTAS_PER_SM 3
+
+__device__ __forceinline__ uint32_t g_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t g_lanemask_lt() {
+    uint32_t m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// plan: tile_count[ntiles] -> tile_off (exclusive scan), tile_cur (= tile_off, the scatter's cursors), items
+// plan_hdr[0] = number of items, [1] = number of entries
+__global__ void __launch_bounds__(1024) k_gather_plan(const uint32_t* __restrict__ tile_count, uint32_t* __restrict__ tile_off,
+                                                      uint32_t* __restrict__ tile_cur, uint4* __restrict__ items,
+                                                      uint32_t* __restrict__ plan_hdr, uint32_t ntiles) {
+    __shared__ unsigned long long wsum[32];
+    __shared__ unsigned long long carry_s;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (uint32_t t0 = 0; t0 < ntiles; t0 += 4096) {
+        const uint32_t i = t0 + threadIdx.x * 4;
+        uint32_t c[4];
+        unsigned long long s = 0;                       // hi 32 bits: entries, lo 32 bits: items
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            c[k] = (i + k < ntiles) ? tile_count[i + k] : 0u;
+            s += ((unsigned long long)c[k] << 32) | (unsigned long long)((c[k] + IG_GCH - 1) / IG_GCH);
+        }
+        unsigned long long inc = s;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            unsigned long long y = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += y;
+        }
+        if (lane == 31) wsum[warp] = inc;
+        __syncthreads();
+        if (warp == 0) {
+            unsigned long long w = wsum[lane], wi = w;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                unsigned long long y = __shfl_up_sync(0xffffffffu, wi, o);
+                if (lane >= o) wi += y;
+            }
+            wsum[lane] = wi - w;
+        }
+        __syncthreads();
+        const unsigned long long carry = carry_s;
+        unsigned long long ex = carry + wsum[warp] + (inc - s);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (i + k < ntiles) {
+                const uint32_t off = (uint32_t)(ex >> 32), ioff = (uint32_t)ex;
+                tile_off[i + k] = off;
+                tile_cur[i + k] = off;
+                for (uint32_t j = 0, left = c[k]; left; ++j) {
+                    const uint32_t n = left < IG_GCH ? left : IG_GCH;
+                    items[ioff + j] = make_uint4(i + k, off + j * IG_GCH, n, 0u);
+                    left -= n;
+                }
+            }
+            ex += ((unsigned long long)c[k] << 32) | (unsigned long long)((c[k] + IG_GCH - 1) / IG_GCH);
+        }
+        __syncthreads();
+        if (threadIdx.x == 1023) carry_s = ex;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { plan_hdr[0] = (uint32_t)carry_s; plan_hdr[1] = (uint32_t)(carry_s >> 32); }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// scatter: one warp per work item of the record stream (IG_CH records); marked records go to their tile's list.
+// Entry (16 + 16 * NPOL bytes): header {ox, oy, S, kbase} (footprint origin relative to the origin tile) followed per
+// polarisation by {v_re, v_re, -v_im, v_im}: the two operand pairs of the packed complex multiply-accumulate, so that
+// the gridder's shared-memory loads deliver them as aligned register pairs with no arithmetic.
+template <int NPOL>
+__global__ void __launch_bounds__(256) k_gather_scatter(const char* __restrict__ records, const uint32_t* __restrict__ gcount,
+                                                        long long n_chunks, uint32_t* __restrict__ tile_cur, int tiles_x,
+                                                        char* __restrict__ entries) {
+    constexpr int STRIDE = NPOL == 4 ? 48 : 32;
+    constexpr int GSTRIDE = 16 + 16 * NPOL;
+    const long long chunk = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (chunk >= n_chunks || gcount[chunk] == 0) return;
+    for (int g = 0; g < IG_CH / 32; ++g) {
+        const char* rec = records + ((size_t)chunk * IG_CH + g * 32 + lane) * STRIDE;
+        const uint4 h = *reinterpret_cast<const uint4*>(rec);
+        const bool mine = (h.z & IG_HDR_GATHER) && !(h.z & IG_HDR_MERGED);
+        const uint32_t gm = __ballot_sync(0xffffffffu, mine);
+        if (!gm) continue;
+        if (mine) {
+            const int X0 = (int)(h.x & 0xffffu), Y0 = (int)(h.x >> 16);
+            const uint32_t tile = (uint32_t)((Y0 >> IG_GT_SHIFT) * tiles_x + (X0 >> IG_GT_SHIFT));
+            const uint32_t peers = __match_any_sync(gm, tile);
+            const int leader = __ffs(peers) - 1;
+            uint32_t base = 0;
+            if (lane == leader) base = atomicAdd(&tile_cur[tile], (uint32_t)__popc(peers));
+            base = __shfl_sync(peers, base, leader);
+            char* e = entries + (size_t)(base + __popc(peers & g_lanemask_lt())) * GSTRIDE;
+            *reinterpret_cast<uint4*>(e) = make_uint4((uint32_t)(X0 & (IG_GT - 1)), (uint32_t)(Y0 & (IG_GT - 1)), h.w, h.y);
+            float v[8];
+            const float4 a = *reinterpret_cast<const float4*>(rec + 16);
+            v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w;
+            if constexpr (NPOL == 4) {
+                const float4 c = *reinterpret_cast<const float4*>(rec + 32);
+                v[4] = c.x; v[5] = c.y; v[6] = c.z; v[7] = c.w;
+            }
+#pragma unroll
+            for (int q = 0; q < NPOL; ++q)
+                *reinterpret_cast<float4*>(e + 16 + 16 * q) = make_float4(v[2 * q], v[2 * q], -v[2 * q + 1], v[2 * q + 1]);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+typedef unsigned long long gf32x2;
+__device__ __forceinline__ void g_unpack2(gf32x2 v, float& lo, float& hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+
+// One row group (4 rows of the sub-tile, one pixel per lane) of one record, as ONE PTX block so that the sums stay in
+// place and no branch is needed: p = this lane's pixel lies inside the footprint (ty = ty0 + 4K in [0, S); lanes
+// outside the footprint's columns carry ty0 = 2^30); the kernel value is a predicated read-only load and ZERO outside
+// the footprint, so the FMAs run unpredicated (FFMA2 has no predicated form: ptxas turns "@p fma.f32x2" into FFMA2 + 2 SEL);
+// per polarisation acc += (v_re,v_re)*(k_re,k_im); acc += (-v_im,v_im)*(k_im,k_re)   (two packed FMAs, SASS FFMA2).
+template <int K>
+__device__ __forceinline__ void g_rowgroup(gf32x2 (&acc)[4], const gf32x2 (&vre)[4], const gf32x2 (&vim)[4], int ty0, int S,
+                                           const unsigned long long* base, unsigned stride_bytes) {
+    asm volatile("{\n\t.reg .pred p;\n\t.reg .b64 kv, ks, ad;\n\t.reg .f32 kr, ki;\n\t.reg .s32 t;\n\t"
+                 "add.s32 t, %4, %8;\n\t"
+                 "setp.lt.u32 p, t, %5;\n\t"
+                 "mad.wide.u32 ad, %6, %9, %7;\n\t"
+                 "mov.b64 kv, 0;\n\t@p ld.global.nc.b64 kv, [ad];\n\t"
+                 "mov.b64 {kr, ki}, kv;\n\t"
+                 "mov.b64 ks, {ki, kr};\n\t"
+                 "fma.rn.f32x2 %0, %10, kv, %0;\n\tfma.rn.f32x2 %1, %12, kv, %1;\n\t"
+                 "fma.rn.f32x2 %2, %14, kv, %2;\n\tfma.rn.f32x2 %3, %16, kv, %3;\n\t"
+                 "fma.rn.f32x2 %0, %11, ks, %0;\n\tfma.rn.f32x2 %1, %13, ks, %1;\n\t"
+                 "fma.rn.f32x2 %2, %15, ks, %2;\n\tfma.rn.f32x2 %3, %17, ks, %3;\n\t}"
+                 : "+l"(acc[0]), "+l"(acc[1]), "+l"(acc[2]), "+l"(acc[3])
+                 : "r"(ty0), "r"(S), "r"(stride_bytes), "l"(base), "n"(4 * K), "n"(K),
+                   "l"(vre[0]), "l"(vim[0]), "l"(vre[1]), "l"(vim[1]), "l"(vre[2]), "l"(vim[2]), "l"(vre[3]), "l"(vim[3]));
+}
+template <int K>
+__device__ __forceinline__ void g_rowgroup(gf32x2 (&acc)[2], const gf32x2 (&vre)[2], const gf32x2 (&vim)[2], int ty0, int S,
+                                           const unsigned long long* base, unsigned stride_bytes) {
+    asm volatile("{\n\t.reg .pred p;\n\t.reg .b64 kv, ks, ad;\n\t.reg .f32 kr, ki;\n\t.reg .s32 t;\n\t"
+                 "add.s32 t, %2, %6;\n\t"
+                 "setp.lt.u32 p, t, %3;\n\t"
+                 "mad.wide.u32 ad, %4, %7, %5;\n\t"
+                 "mov.b64 kv, 0;\n\t@p ld.global.nc.b64 kv, [ad];\n\t"
+                 "mov.b64 {kr, ki}, kv;\n\t"
+                 "mov.b64 ks, {ki, kr};\n\t"
+                 "fma.rn.f32x2 %0, %8, kv, %0;\n\tfma.rn.f32x2 %1, %10, kv, %1;\n\t"
+                 "fma.rn.f32x2 %0, %9, ks, %0;\n\tfma.rn.f32x2 %1, %11, ks, %1;\n\t}"
+                 : "+l"(acc[0]), "+l"(acc[1])
+                 : "r"(ty0), "r"(S), "r"(stride_bytes), "l"(base), "n"(4 * K), "n"(K),
+                   "l"(vre[0]), "l"(vim[0]), "l"(vre[1]), "l"(vim[1]));
+}
+template <int K>
+__device__ __forceinline__ void g_rowgroup(gf32x2 (&acc)[1], const gf32x2 (&vre)[1], const gf32x2 (&vim)[1], int ty0, int S,
+                                           const unsigned long long* base, unsigned stride_bytes) {
+    asm volatile("{\n\t.reg .pred p;\n\t.reg .b64 kv, ks, ad;\n\t.reg .f32 kr, ki;\n\t.reg .s32 t;\n\t"
+                 "add.s32 t, %1, %5;\n\t"
+                 "setp.lt.u32 p, t, %2;\n\t"
+                 "mad.wide.u32 ad, %3, %6, %4;\n\t"
+                 "mov.b64 kv, 0;\n\t@p ld.global.nc.b64 kv, [ad];\n\t"
+                 "mov.b64 {kr, ki}, kv;\n\t"
+                 "mov.b64 ks, {ki, kr};\n\t"
+                 "fma.rn.f32x2 %0, %7, kv, %0;\n\t"
+                 "fma.rn.f32x2 %0, %8, ks, %0;\n\t}"
+                 : "+l"(acc[0])
+                 : "r"(ty0), "r"(S), "r"(stride_bytes), "l"(base), "n"(4 * K), "n"(K), "l"(vre[0]), "l"(vim[0]));
+}
+
+template <int NPOL, bool COUNT>
+__global__ void __launch_bounds__(IG_GW * 32, IG_GCTAS_PER_SM)
+k_gather(const char* __restrict__ entries, const uint4* __restrict__ items, const uint32_t* __restrict__ plan_hdr,
+         float* __restrict__ grid, const float2* __restrict__ bank, int N, int tiles_x, unsigned* __restrict__ ticket,
+         unsigned long long* __restrict__ commits) {
+    constexpr int GSTRIDE = 16 + 16 * NPOL;
+    __shared__ __align__(128) char buf[IG_GCH * GSTRIDE];
+    __shared__ __align__(8) uint64_t bar;
+    __shared__ unsigned s_item, s_sub;
+    const int lane = threadIdx.x & 31;
+    const int lx = lane & 7, lr = lane >> 3;
+    const unsigned n_items = plan_hdr[0];
+    const unsigned long long plane_bytes = (unsigned long long)N * N * 16;   // 4 pol: two planes of pol pairs
+    const unsigned long long* __restrict__ bank64 = reinterpret_cast<const unsigned long long*>(bank);
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(g_smem_u32(&bar)), "r"(1) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    uint32_t phase = 0;
+    unsigned n_commit = 0;
+    for (;;) {
+        __syncthreads();                                   // every warp is done with buf, s_item, s_sub
+        if (threadIdx.x == 0) { s_item = atomicAdd(ticket, 1u); s_sub = 0; }
+        __syncthreads();
+        const unsigned it = s_item;
+        if (it >= n_items) break;
+        const uint4 item = items[it];                      // {tile, first entry, entries, -}
+        const int count = (int)item.z;
+        if (threadIdx.x == 0) {
+            const uint32_t bytes = (uint32_t)count * GSTRIDE;
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic reads of buf before the async write
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(g_smem_u32(&bar)), "r"(bytes) : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(g_smem_u32(buf)),
+                         "l"(entries + (size_t)item.y * GSTRIDE), "r"(bytes), "r"(g_smem_u32(&bar))
+                         : "memory");
+        }
+        asm volatile(
+            "{\n.reg .pred p;\nGW_%=:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra GD_%=;\nbra GW_%=;\nGD_%=:\n}\n" ::"r"(
+                g_smem_u32(&bar)),
+            "r"(phase)
+            : "memory");
+        phase ^= 1u;
+        // largest support of the item -> the region its footprints can reach from the origin tile
+        int smax = 0;
+        for (int e = lane; e < count; e += 32) smax = max(smax, *reinterpret_cast<const int*>(buf + e * GSTRIDE + 8));
+        smax = __reduce_max_sync(0xffffffffu, smax);
+        const int nsx = (IG_GT - 1 + smax + 7) >> 3, nsy = (IG_GT - 1 + smax + 4 * IG_GR - 1) / (4 * IG_GR);
+        const unsigned nsub = (unsigned)(nsx * nsy);
+        const int tile_y = (int)item.x / tiles_x, tile_x = (int)item.x - tile_y * tiles_x;
+        for (;;) {
+            unsigned st = 0;
+            if (lane == 0) st = atomicAdd(&s_sub, 1u);
+            st = __shfl_sync(0xffffffffu, st, 0);
+            if (st >= nsub) break;
+            const int sy = (int)st / nsx, sx = (int)st - sy * nsx;
+            const int sub_x = sx * 8, sub_y = sy * (4 * IG_GR);        // sub-tile origin relative to the origin tile
+            gf32x2 acc[IG_GR][NPOL];
+#pragma unroll
+            for (int k = 0; k < IG_GR; ++k)
+#pragma unroll
+                for (int q = 0; q < NPOL; ++q) acc[k][q] = 0ull;
+            for (int g0 = 0; g0 < count; g0 += 32) {
+                // which of these 32 records touch the sub-tile: footprint [ox, ox+S) x [oy, oy+S) against [sub_x, sub_x+8) x [sub_y, sub_y+16)
+                bool hit = false;
+                if (g0 + lane < count) {
+                    const int4 w = *reinterpret_cast<const int4*>(buf + (g0 + lane) * GSTRIDE);
+                    const int ox = w.x - sub_x, oy = w.y - sub_y;
+                    hit = ox < 8 && ox + w.z > 0 && oy < 4 * IG_GR && oy + w.z > 0;
+                }
+                uint32_t m = __ballot_sync(0xffffffffu, hit);
+                while (m) {
+                    const int b = __ffs(m) - 1;
+                    m &= m - 1;
+                    const char* ep = buf + (g0 + b) * GSTRIDE;
+                    const int4 h = *reinterpret_cast<const int4*>(ep);              // warp-wide broadcast: {ox, oy, S, kbase}
+                    gf32x2 vre[NPOL], vim[NPOL];
+#pragma unroll
+                    for (int q = 0; q < NPOL; ++q) {
+                        const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(ep + 16 + 16 * q);
+                        vre[q] = t.x; vim[q] = t.y;
+                    }
+                    const int S = h.z;
+                    const int tx = lx - (h.x - sub_x);                               // this lane's tap column
+                    const int ty = lr - (h.y - sub_y);                               // tap row of row group 0
+                    const int ty0 = (unsigned)tx < (unsigned)S ? ty : (1 << 30);     // columns outside the footprint never pass
+                    const unsigned long long* base = bank64 + (long long)(uint32_t)h.w + (long long)(ty * S + tx);
+                    const unsigned stride = 32u * (unsigned)S;                        // 4 rows of S taps of 8 bytes
+                    g_rowgroup<0>(acc[0], vre, vim, ty0, S, base, stride);
+                    g_rowgroup<1>(acc[1], vre, vim, ty0, S, base, stride);
+                    g_rowgroup<2>(acc[2], vre, vim, ty0, S, base, stride);
+                    g_rowgroup<3>(acc[3], vre, vim, ty0, S, base, stride);
+                }
+            }
+            // write the sub-tile: one vector reduction per touched pixel and polarisation pair (other items, and the
+            // moving-window gridder, add to the same grid)
+            const int x = (tile_x << IG_GT_SHIFT) + sub_x + lx;
+#pragma unroll
+            for (int k = 0; k < IG_GR; ++k) {
+                const int y = (tile_y << IG_GT_SHIFT) + sub_y + 4 * k + lr;
+                gf32x2 any = 0ull;
+#pragma unroll
+                for (int q = 0; q < NPOL; ++q) any |= acc[k][q];
+                if (any != 0ull && x < N && y < N) {
+                    const size_t pix = (size_t)y * N + x;
+                    float a[2 * NPOL];
+#pragma unroll
+                    for (int q = 0; q < NPOL; ++q) g_unpack2(acc[k][q], a[2 * q], a[2 * q + 1]);
+                    if constexpr (NPOL == 1) {
+                        asm volatile("red.global.add.v2.f32 [%0], {%1,%2};" ::"l"(grid + pix * 2), "f"(a[0]), "f"(a[1]) : "memory");
+                    } else {
+                        float* gp = grid + pix * 4;
+                        asm volatile("red.global.add.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(gp), "f"(a[0]), "f"(a[1]), "f"(a[2]), "f"(a[3]) : "memory");
+                        if constexpr (NPOL == 4) {
+                            float* g2 = reinterpret_cast<float*>(reinterpret_cast<char*>(gp) + plane_bytes);
+                            asm volatile("red.global.add.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(g2), "f"(a[4]), "f"(a[5]), "f"(a[6]), "f"(a[7]) : "memory");
+                        }
+                    }
+                    if constexpr (COUNT) ++n_commit;
+                }
+            }
+        }
+    }
+    if constexpr (COUNT) {
+        n_commit = __reduce_add_sync(0xffffffffu, n_commit);
+        if (lane == 0 && n_commit) atomicAdd(commits, (unsigned long long)n_commit);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+size_t ig_gather_tiles(const ig_ctx* c) {
+    const size_t t = (size_t)((c->prm.N + IG_GT - 1) / IG_GT);
+    return t * t;
+}
+size_t ig_gather_max_items(const ig_ctx* c, long long n_chunks) {
+    return (size_t)n_chunks * IG_CH / IG_GCH + ig_gather_tiles(c) + 1;
+}
+
+int ig_launch_gather(ig_ctx* c, const char* records, const uint32_t* gcount, long long n_chunks, uint32_t* tile_count,
+                     uint32_t* tile_off, uint32_t* tile_cur, uint4* items, uint32_t* plan_hdr, char* entries) {
+    if (n_chunks == 0) return 0;
+    const uint32_t ntiles = (uint32_t)ig_gather_tiles(c);
+    const int tiles_x = (c->prm.N + IG_GT - 1) / IG_GT;
+    k_gather_plan<<<1, 1024, 0, c->stream>>>(tile_count, tile_off, tile_cur, items, plan_hdr, ntiles);
+    const unsigned sblocks = (unsigned)((n_chunks + 7) / 8);
+    switch (c->prm.npol) {
+        case 1: k_gather_scatter<1><<<sblocks, 256, 0, c->stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, entries); break;
+        case 2: k_gather_scatter<2><<<sblocks, 256, 0, c->stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, entries); break;
+        default: k_gather_scatter<4><<<sblocks, 256, 0, c->stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, entries); break;
+    }
+    IG_CUDA_OK(c, cudaMemsetAsync(&c->d_acc->ticket, 0, sizeof(unsigned), c->stream));
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    dim3 g((unsigned)(sms * IG_GCTAS_PER_SM)), b(IG_GW * 32);
+#define IG_GLAUNCH(P, C) k_gather<P, C><<<g, b, 0, c->stream>>>(entries, items, plan_hdr, c->grid, c->d_bank, c->prm.N, tiles_x, &c->d_acc->ticket, &c->d_acc->commits)
+    if (c->count_commits) {
+        switch (c->prm.npol) { case 1: IG_GLAUNCH(1, true); break; case 2: IG_GLAUNCH(2, true); break; default: IG_GLAUNCH(4, true); break; }
+    } else {
+        switch (c->prm.npol) { case 1: IG_GLAUNCH(1, false); break; case 2: IG_GLAUNCH(2, false); break; default: IG_GLAUNCH(4, false); break; }
+    }
+#undef IG_GLAUNCH
+    IG_CUDA_OK(c, cudaGetLastError());
+    return 3;
+}

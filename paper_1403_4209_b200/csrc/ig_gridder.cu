@@ -185,13 +185,13 @@ __device__ __forceinline__ unsigned grid_run(const char* __restrict__ rp, int n_
         // Same window as the record before (same cell; only the sub-cell offsets, hence the kernel matrix,
         // may differ): every lane keeps its pixels and taps, so the index arithmetic and the commit test
         // are skipped. Slow baselines stay in a cell for many records (warp-uniform branch).
-        const bool same = (h.x == last_x) && ((h.z & 0x00ffffffu) == last_z);
+        const bool same = (h.x == last_x) && ((h.z & IG_HDR_WINDOW) == last_z);
         if (same) {
 #pragma unroll
             for (int k = 0; k < R; ++k) kv[k] = __ldg(bank64 + (uint32_t)(krel[k] + h.y));
         } else {
-            last_x = h.x; last_z = h.z & 0x00ffffffu;
-            const int cm = (int)(h.z & 0xffu), dm = (int)((h.z >> 8) & 0xffu);
+            last_x = h.x; last_z = h.z & IG_HDR_WINDOW;
+            const int cm = IG_HDR_C(h.z), dm = IG_HDR_D(h.z);
             int pix[R];
 #pragma unroll
             for (int k = 0; k < R; ++k) {
@@ -271,7 +271,7 @@ k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_s
 #pragma unroll
         for (int g = 0; g < IG_NSTAGE; ++g) {
             mbar_wait(&my_bar[g], phase);
-            const int sv = (int)((*reinterpret_cast<const uint32_t*>(my_rec + (g * 32 + lane) * STRIDE + 8) >> 16) & 0xffu);
+            const int sv = IG_HDR_S(*reinterpret_cast<const uint32_t*>(my_rec + (g * 32 + lane) * STRIDE + 8));
             int before = __shfl_up_sync(0xffffffffu, sv, 1);
             if (lane == 0) before = s_prev;
             bnd[g] = __ballot_sync(0xffffffffu, sv != before);
@@ -290,7 +290,7 @@ k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_s
                 if (m) r1 = g * 32 + __ffs(m) - 1;     // lower words are visited last: smallest wins
             }
             const char* rp = my_rec + r0 * STRIDE;
-            const int S = (int)((*reinterpret_cast<const uint32_t*>(rp + 8) >> 16) & 0xffu);
+            const int S = IG_HDR_S(*reinterpret_cast<const uint32_t*>(rp + 8));
             if (S != 0) {
                 const int s2 = S * S;
                 const int n_pass = (s2 + 32 * IG_RMAX - 1) / (32 * IG_RMAX);

@@ -30,6 +30,11 @@ __device__ __forceinline__ IgIndex ig_index_one(const IgParams& P, const IgPlane
     IgIndex r;
     double fu = __dmul_rn(__dmul_rn(um, nu), P.ku);
     double fv = __dmul_rn(__dmul_rn(vm, nu), P.ku);
+    double wl = __dmul_rn(wm, nu);
+    // a non-finite coordinate has no cell: the record is dropped (reading 20). Decided before any integer conversion
+    // or table lookup; the tuple of such a record is all zero apart from the conj bit
+    const bool finite = isfinite(fu) && isfinite(fv) && isfinite(wl);
+    if (!finite) { fu = 0.0; fv = 0.0; wl = 0.0; }
     long long U = (long long)ceil(__dsub_rn(fu, 0.5));   // nearest sample, ties towards -inf
     long long V = (long long)ceil(__dsub_rn(fv, 0.5));
     long long x, y;                                      // -du/2 < delta <= du/2 (eq 4.2)
@@ -49,7 +54,7 @@ __device__ __forceinline__ IgIndex ig_index_one(const IgParams& P, const IgPlane
     r.ov = (int)(V - y * P.beta);
     int p = 0;
     if (P.P > 1) {
-        double sp = floor(__dadd_rn(__dsqrt_rn(__dmul_rn(__dmul_rn(wm, nu), P.kw)), 0.5));
+        double sp = floor(__dadd_rn(__dsqrt_rn(__dmul_rn(wl, P.kw)), 0.5));
         p = sp >= (double)(P.P - 1) ? P.P - 1 : (int)sp;
     }
     r.p = p;
@@ -57,6 +62,7 @@ __device__ __forceinline__ IgIndex ig_index_one(const IgParams& P, const IgPlane
     long long h = (r.S - 1) / 2;
     long long Xc = x + P.N / 2, Yc = y + P.N / 2;
     r.on = (Xc - h >= 0) && (Xc + h <= P.N - 1) && (Yc - h >= 0) && (Yc + h <= P.N - 1);
+    if (!finite) { r.on = 0; r.ou = r.ov = 0; Xc = Yc = 0; r.p = 0; r.S = planes[0].support; }
     const long long lim = 1ll << 30;
     Xc = Xc < -lim ? -lim : (Xc > lim ? lim : Xc);
     Yc = Yc < -lim ? -lim : (Yc > lim ? lim : Yc);
@@ -65,7 +71,7 @@ __device__ __forceinline__ IgIndex ig_index_one(const IgParams& P, const IgPlane
 }
 
 // One CTA = one row block of IG_CH sorted rows; thread t = row rb*IG_CH + t; loop over channels.
-// Record at place ((rb*nchan + c)*IG_CH + t): 16-byte header {pix_base, kbase, c|d<<8|S<<16|conj<<24, plane}
+// Record at place ((rb*nchan + c)*IG_CH + t): 16-byte header {pix_base, kbase, z = c | d<<9 | S<<18 | flags (ig_internal.h), plane}
 // followed by npol complex32 pairs (stride 48 B for 4 pol, else 32 B).
 template <int NPOL>
 __global__ void __launch_bounds__(IG_CH)
@@ -73,7 +79,8 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
         const double* __restrict__ uvw, const uint32_t* __restrict__ perm, long long nrow,
         const double* __restrict__ freqs, int nchan, const float* __restrict__ vis,
         const float* __restrict__ wt, char* __restrict__ records, uint32_t* __restrict__ chunk_smax,
-        IgAccum* __restrict__ acc, bool compress, double* __restrict__ chan_norm) {
+        IgAccum* __restrict__ acc, bool compress, double* __restrict__ chan_norm,
+        uint32_t* __restrict__ gcount, uint32_t* __restrict__ tile_count, int gather_min, int tiles_x) {
     constexpr int STRIDE = NPOL == 4 ? 48 : 32;
     const long long rb = blockIdx.x;
     const int t = threadIdx.x, lane = t & 31;
@@ -120,6 +127,8 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
 #pragma unroll
         for (int q = 0; q < 2 * NPOL; ++q) v[q] = 0.f;
         int S = 0;
+        bool is_g = false;                // large support: goes to the gather gridder (ig_gather.cu)
+        uint32_t g_tile = 0;
         double cn[NPOL];                  // this record's normaliser terms (per-channel grid mode)
 #pragma unroll
         for (int q = 0; q < NPOL; ++q) cn[q] = 0.0;
@@ -148,10 +157,18 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
                 int cm = (-a0) % S; if (cm < 0) cm += S;
                 int dm = (-b0) % S; if (dm < 0) dm += S;
                 const uint32_t tab = (uint32_t)((ix.ov + P.shift) * P.beta + (ix.ou + P.shift));
-                hdr.x = (uint32_t)(b0 * P.N + a0);
                 hdr.y = planes[ix.p].koff + tab * (uint32_t)(S * S);
-                hdr.z = (uint32_t)cm | ((uint32_t)dm << 8) | ((uint32_t)S << 16) | ((uint32_t)conj << 24);
-                hdr.w = (uint32_t)ix.p;
+                is_g = S >= gather_min;
+                if (is_g) {
+                    hdr.x = (uint32_t)a0 | ((uint32_t)b0 << 16);
+                    hdr.z = IG_HDR_GATHER | (conj ? IG_HDR_CONJ : 0u);
+                    hdr.w = (uint32_t)S;
+                    g_tile = (uint32_t)((b0 >> 5) * tiles_x + (a0 >> 5));     // origin tile, 32 x 32 pixels
+                } else {
+                    hdr.x = (uint32_t)(b0 * P.N + a0);
+                    hdr.z = IG_HDR_PACK(cm, dm, S) | (conj ? IG_HDR_CONJ : 0u);
+                    hdr.w = (uint32_t)ix.p;
+                }
                 const double z = zeta[(size_t)ix.p * P.beta * P.beta + tab];
 #pragma unroll
                 for (int q = 0; q < NPOL; ++q) {
@@ -212,7 +229,17 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
                 if (lane == 0 && x != 0.0) atomicAdd(&chan_norm[(size_t)c * 4 + q], x);
             }
         }
-        unsigned smax = __reduce_max_sync(0xffffffffu, (unsigned)S);
+        // plan of the gather gridder: marked records per origin tile (warp-aggregated) and per work item
+        const bool count_me = is_g && !(hdr.z & IG_HDR_MERGED);
+        const uint32_t gm = __ballot_sync(0xffffffffu, count_me);
+        if (gm) {
+            if (count_me) {
+                const uint32_t peers = __match_any_sync(gm, g_tile);
+                if (lane == __ffs(peers) - 1) atomicAdd(&tile_count[g_tile], (uint32_t)__popc(peers));
+            }
+            if (lane == 0) atomicAdd(&gcount[chunk], (uint32_t)__popc(gm));
+        }
+        unsigned smax = __reduce_max_sync(0xffffffffu, is_g ? 0u : (unsigned)S);
         if (lane == 0 && smax) atomicMax(&chunk_smax[chunk], smax);
       }
     }
@@ -261,17 +288,23 @@ __global__ void k_debug_index(IgParams P, const IgPlaneEntry* __restrict__ plane
 }
 
 int ig_launch_index(ig_ctx* c, const double* uvw, const uint32_t* perm, long long nrow, const double* d_freqs,
-                    int nchan, const float* vis, const float* wt, char* records, uint32_t* chunk_smax) {
+                    int nchan, const float* vis, const float* wt, char* records, uint32_t* chunk_smax, uint32_t* gcount,
+                    uint32_t* tile_count, int gather_min) {
     long long nrb = (nrow + IG_CH - 1) / IG_CH;
     if (nrb == 0) return 0;
     if (nrb > 0x7fffffffll) { c->err = "too many rows"; return -1; }
-    IG_CUDA_OK(c, cudaMemsetAsync(chunk_smax, 0, (size_t)nrb * nchan * 4, c->stream));
+    // chunk_smax and gcount are neighbours in the work buffer: one memset clears both
+    IG_CUDA_OK(c, cudaMemsetAsync(chunk_smax, 0, (size_t)((char*)(gcount + nrb * nchan) - (char*)chunk_smax), c->stream));
+    IG_CUDA_OK(c, cudaMemsetAsync(tile_count, 0, ig_gather_tiles(c) * 4, c->stream));
     dim3 g((unsigned)nrb), b(IG_CH);
+    const int tiles_x = (c->prm.N + 31) / 32;
+#define IG_INDEX(P_) k_index<P_><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc, c->compress, c->per_channel ? c->d_chan_norm : nullptr, gcount, tile_count, gather_min, tiles_x)
     switch (c->prm.npol) {
-        case 1: k_index<1><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc, c->compress, c->per_channel ? c->d_chan_norm : nullptr); break;
-        case 2: k_index<2><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc, c->compress, c->per_channel ? c->d_chan_norm : nullptr); break;
-        default: k_index<4><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc, c->compress, c->per_channel ? c->d_chan_norm : nullptr); break;
+        case 1: IG_INDEX(1); break;
+        case 2: IG_INDEX(2); break;
+        default: IG_INDEX(4); break;
     }
+#undef IG_INDEX
     IG_CUDA_OK(c, cudaGetLastError());
     return 1;
 }

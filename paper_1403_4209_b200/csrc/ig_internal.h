@@ -18,7 +18,19 @@
 #define IG_GRID_CTAS_PER_SM 5
 #endif
 // IG_GRID_CTAS_PER_SM: launch bound and persistent grid size
-#define IG_HDR_MERGED (1u << 25)   // record header word z: visibility already summed into the run's head record
+// Record header word z (16-byte header {pix_base, kbase, z, plane}): Romein offsets c, d (eq 4.7) and the
+// support S in 9 bits each (S <= 511, the largest support the thesis sweeps), then flags.
+#define IG_HDR_C(z) ((int)((z) & 0x1ffu))
+#define IG_HDR_D(z) ((int)(((z) >> 9) & 0x1ffu))
+#define IG_HDR_S(z) ((int)(((z) >> 18) & 0x1ffu))
+#define IG_HDR_PACK(c, d, S) ((uint32_t)(c) | ((uint32_t)(d) << 9) | ((uint32_t)(S) << 18))
+#define IG_HDR_WINDOW 0x07ffffffu  // c, d, S: with pix_base, the window a record's footprint occupies
+#define IG_HDR_CONJ (1u << 27)     // visibility was conjugated (w < 0, eq 4.10)
+#define IG_HDR_MERGED (1u << 28)   // visibility already summed into the run's head record (compression)
+// Large-support record that the fixed-tile gather gridder handles (ig_gather.cu). Its header is
+// {X0 | Y0 << 16, kbase, flags (c = d = S = 0, so the moving-window gridder sees a skip record), S}.
+#define IG_HDR_GATHER (1u << 29)
+#define IG_GATHER_MIN_DEFAULT 17   // supports >= this go to the gather gridder (ig_set_gather_min_support)
 #define IG_MAX_CHAN_GRIDS 4096   // per-channel grid mode: channels whose normalisers the bank head has room for
 #define IG_GRID_WARPS 4      // warps per gridder CTA
 
@@ -55,6 +67,8 @@ struct ig_ctx {
     bool per_channel = false;                 // ig_set_per_channel_grids: one grid per channel (thesis default, :1120)
     double* d_chan_norm = nullptr;            // [IG_MAX_CHAN_GRIDS][4] normalisers of the per-channel grids
     bool compress = true;                     // ig_set_compression
+    int tile_shift = 0;                       // ig_set_sort_tile_shift (0 = automatic: N/8 cells, at least 128)
+    int gather_min = IG_GATHER_MIN_DEFAULT;   // ig_set_gather_min_support
     bool count_commits = false;               // ig_set_commit_counting
     // bank description (host copies)
     std::vector<int> support;
@@ -83,7 +97,12 @@ size_t ig_sort_scratch_bytes(long long nrow);
 // (compression is applied in k_index when c->compress is set)
 int ig_launch_index(ig_ctx* c, const double* uvw, const uint32_t* perm, long long nrow,
                     const double* d_freqs, int nchan, const float* vis, const float* wt,
-                    char* records, uint32_t* chunk_smax);   // uses c->per_channel / c->d_chan_norm
+                    char* records, uint32_t* chunk_smax, uint32_t* gcount, uint32_t* tile_count, int gather_min);   // uses c->per_channel / c->d_chan_norm
+// gather gridder (ig_gather.cu): plan, scatter, gridder; gcount[chunk] = marked records per work item
+size_t ig_gather_tiles(const ig_ctx* c);
+size_t ig_gather_max_items(const ig_ctx* c, long long n_chunks);
+int ig_launch_gather(ig_ctx* c, const char* records, const uint32_t* gcount, long long n_chunks, uint32_t* tile_count,
+                     uint32_t* tile_off, uint32_t* tile_cur, uint4* items, uint32_t* plan_hdr, char* entries);
 int ig_launch_debug_index(ig_ctx* c, const double* uvw, long long nrow, const double* d_freqs, int nchan,
                           int* X, int* Y, int* ou, int* ov, int* pl, int* fl);
 int ig_launch_gridder(ig_ctx* c, const char* records, const uint32_t* chunk_smax, long long nrb, int nchan);

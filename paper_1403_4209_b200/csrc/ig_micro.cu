@@ -41,14 +41,13 @@ __global__ void __launch_bounds__(256) k_ffma2_peak(float* out, int iters, float
     if (s == 0x123456789ull) out[0] = 1.f;
 }
 
-extern "C" ig_status ig_measure_fp32_peak(void* cuda_stream, double* tflops) {
-    if (!tflops) return IG_EINVAL;
+extern "C" ig_status ig_measure_fp32_peak(void* cuda_stream, void* sink_dev, double* tflops) {
+    if (!tflops || !sink_dev) return IG_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
         return IG_ECUDA;
-    float* d = nullptr;   // 4-byte sink, only ever written if the impossible branch is taken
-    if (cudaMalloc(&d, 4) != cudaSuccess) return IG_ECUDA;
+    float* d = (float*)sink_dev;   // caller's 4-byte sink, only ever written if the impossible branch is taken
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0); cudaEventCreate(&e1);
     const int iters = 20000, ctas = sms * 8, thr = 256;
@@ -58,7 +57,7 @@ extern "C" ig_status ig_measure_fp32_peak(void* cuda_stream, double* tflops) {
         if (rep & 1) k_ffma2_peak<<<ctas, thr, 0, st>>>(d, iters / 2, 1.0000001f, 1e-9f);
         else k_ffma_peak<<<ctas, thr, 0, st>>>(d, iters, 1.0000001f, 1e-9f);
         cudaEventRecord(e1, st);
-        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d); return IG_ECUDA; }
+        if (cudaEventSynchronize(e1) != cudaSuccess) return IG_ECUDA;
         float ms = 0;
         cudaEventElapsedTime(&ms, e0, e1);
         double fl = 2.0 * 64.0 * iters * (double)ctas * thr;
@@ -66,7 +65,6 @@ extern "C" ig_status ig_measure_fp32_peak(void* cuda_stream, double* tflops) {
         if (rep > 1 && t > best) best = t;
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1);
-    cudaFree(d);
     *tflops = best;
     return IG_OK;
 }

@@ -12,7 +12,6 @@
 // r01_v0_gridder.md: 1.0 TB of DRAM traffic on config 5 for 24 M touched pixels). A track
 // that crosses a tile edge is cut there, which costs one flush of the lane registers.
 // Output: perm[j] = input row at sorted place j.
-#include <stdlib.h>
 #include "ig_internal.h"
 
 #define SORT_THREADS 256
@@ -180,7 +179,7 @@ int ig_launch_sort_rows(ig_ctx* c, const double* uvw, const int* baseline_id, lo
     // concurrently running warps collide on the same pixels
     int tile_shift = 7;
     while ((c->prm.N >> tile_shift) > 8) ++tile_shift;
-    if (const char* e = getenv("IG_TILE_SHIFT")) { int t = atoi(e); if (t >= tile_shift && t <= 15) tile_shift = t; }
+    if (c->tile_shift) tile_shift = c->tile_shift;      // ig_set_sort_tile_shift
     const double cells_per_m = ref_freq_hz * c->prm.ku / (double)c->prm.beta;
     k_sort_keys<<<(unsigned)((nrow + 255) / 256), 256, 0, c->stream>>>(uvw, baseline_id, nrow, cells_per_m, c->prm.N,
                                                                       tile_shift, keysA);

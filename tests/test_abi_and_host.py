@@ -39,6 +39,13 @@ def test_create_validates_arguments(lib):
     for a in bad:
         assert lib.ig_create(ctypes.byref(ctx), *a) == 1, a
         assert not ctx.value
+    # supports up to 511 (the thesis sweeps to 511 and its heavy configuration needs 349, :1785-1789, :1924);
+    # a valid odd support beyond the 9-bit header field is IG_EUNSUPPORTED, not IG_EINVAL
+    assert lib.ig_create(ctypes.byref(ctx), 1024, 1e-4, 4, 8, 513, 4) == 5 and not ctx.value
+    for s_ok in (255, 349, 511):
+        assert lib.ig_create(ctypes.byref(ctx), 1024, 1e-4, 4, 8, s_ok, 4) == 0
+        lib.ig_destroy(ctx)
+        ctx = ctypes.c_void_p()
     assert lib.ig_create(ctypes.byref(ctx), *ok) == 0
     assert lib.ig_grid_bytes(ctx) == 256 * 256 * 4 * 8
     sup = np.array([7, 7, 5, 3], dtype=np.int32)
@@ -54,6 +61,28 @@ def test_create_validates_arguments(lib):
     assert lib.ig_build_wkernels(ctx, 10.0, sup.ctypes.data_as(ctypes.c_void_p)) == 2
     assert lib.ig_grid(ctx, None, None, 0, None, 1, None, None) == 2
     assert b"ig_bind" in lib.ig_last_error(ctx)
+    lib.ig_destroy(ctx)
+
+
+def test_host_staging_size_covers_what_ig_grid_host_carves(lib):
+    """ig_grid_host needs align(workspace(slice rows)) + (1 or 2) staging areas of slice rows; a caller that sizes
+    work_dev as ig_workspace_bytes(nrow) + ig_host_staging_bytes(nrow), as the header says, must always have enough:
+    the formula is re-stated here from the header's description of the staging areas (round 1 returned a spurious
+    IG_ENOMEM for unsliced batches with nrow % 128 != 0)."""
+    ctx = ctypes.c_void_p()
+    assert lib.ig_create(ctypes.byref(ctx), 512, 1e-4, 4, 8, 15, 4) == 0
+    al = lambda x: (x + 255) // 256 * 256
+    for nslices in (1, 3, 8):
+        assert lib.ig_set_host_slices(ctx, nslices) == 0
+        for nrow, nchan in ((1000, 64), (1, 1), (127, 3), (65535, 2), (65536, 2), (100001, 5), (1 << 20, 16)):
+            k = 1 if nrow < 65536 else nslices
+            srows = nrow if k == 1 else min(nrow, (((nrow + k - 1) // k) + 127) // 128 * 128)
+            rec = srows * nchan * 4
+            stage = al(srows * 24) + al(srows * 4) + al(rec * 8) + al(rec * 4)
+            need = al(lib.ig_workspace_bytes(ctx, srows, nchan)) + (2 if srows < nrow else 1) * stage
+            have = lib.ig_workspace_bytes(ctx, nrow, nchan) + lib.ig_host_staging_bytes(ctx, nrow, nchan)
+            assert have >= need, (nslices, nrow, nchan, have, need)
+            assert have <= need + lib.ig_workspace_bytes(ctx, nrow, nchan)     # and no unsliced upper bound any more
     lib.ig_destroy(ctx)
 
 

@@ -124,3 +124,26 @@ def test_edge_records_dropped_whole(orc):
     X = idx["X"][:, 0]
     on = (idx["flags"][:, 0] & 2) != 0
     assert np.array_equal(on, (X >= 3) & (X <= 60))
+
+
+def test_non_finite_coordinates_are_dropped(orc):
+    """DESIGN.md reading 20: a NaN or infinite u, v or w has no cell; the record is off the grid (bit1 clear) and its
+    tuple is zero apart from the conj bit, for every channel; finite neighbours are unaffected (:1278 drop rule)."""
+    n, beta, P = 64, 8, 4
+    good = [1.0, 2.0, 3.0]
+    uvw = np.array([good, [np.nan, 2, 3], [1, np.inf, -3], [1, 2, np.nan], [1, 2, -np.inf], good])
+    idx = orc.index_records(uvw, [3e8, 2e8], n, 1e-3, beta, P, 100.0, [7, 7, 9, 9])
+    for r in (1, 2, 3, 4):
+        for k in ("X", "Y", "off_u", "off_v", "plane"):
+            assert (idx[k][r] == 0).all(), (r, k)
+        assert ((idx["flags"][r] & 2) == 0).all()
+    assert idx["flags"][2, 0] == 1 and idx["flags"][4, 0] == 1 and idx["flags"][1, 0] == 0
+    for k in idx:
+        assert (idx[k][0] == idx[k][5]).all()
+    assert (idx["flags"][0] & 2).all()
+    # and the gridder leaves them out of grid, normaliser and the gridded count
+    vis = np.ones((6, 2, 1), np.complex64); wt = np.ones((6, 2, 1), np.float32)
+    bank = np.ones((49 + 49 + 81 + 81) * beta * beta, dtype=np.complex128)
+    off = np.cumsum([0, 49, 49, 81]) * beta * beta
+    g, nrm, st = orc.grid_records(idx, vis, wt, n, beta, [7, 7, 9, 9], bank, off)
+    assert st[0] == 4 and st[1] == 8
