@@ -134,11 +134,19 @@ ig_status ig_grid_host(ig_ctx* ctx, const double* uvw_m, const int* baseline_id,
 
 /* Algorithm 4.6: inverse FFT per polarisation (uv origin at pixel (N/2,N/2), +j sign,
  * unnormalised, eq 2.8 :516), real part divided by the normaliser (eq 4.5), the taper
- * (eq 2.9) and the sinc of the nearest-sample lookup (eq 2.13). No Stokes conversion.
+ * (eq 2.9) and the sinc of the nearest-sample lookup (eq 2.13). By default the images are the polarisations
+ * themselves; ig_set_stokes_output switches step 2's Stokes conversion on.
  *   image_dev        dev f32 [n_pol][N][N], pixel (N/2,N/2) = phase centre
  *   normaliser_host  HOST f64 [n_pol], receives N_p; may be NULL
  * Uses work_dev (ig_finalize_workspace_bytes()). Synchronises. */
 ig_status ig_finalize(ig_ctx* ctx, float* image_dev, double* normaliser_host);
+
+/* Step 2 of Algorithm 4.6, "convert to multiple-Stokes image and normalise". The paper prints no
+ * formulas; reading 21: the polarisations are the linear-feed correlations in MeasurementSet order (XX, XY, YX, YY)
+ * and, with D_p = image_p / N_p,  I = (D_XX + D_YY)/2, Q = (D_XX - D_YY)/2, U = (D_XY + D_YX)/2, V = (D_XY - D_YX)/(2j)
+ * (n_pol = 2 is (XX, YY) -> I, Q; n_pol = 1 -> I = D_0: "only the stokes that can be calculated", :1660).
+ * With the switch on, ig_finalize / ig_finalize_channel write image_dev[s] = Stokes parameter s (I, Q, U, V order). */
+ig_status ig_set_stokes_output(ig_ctx* ctx, int on);
 
 /* Step C runs two work distributions: records with support < s keep Romein's moving window
  * (registers follow a track, atomics when a pixel leaves the window, :710-742); records with support >= s go to

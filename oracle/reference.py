@@ -250,8 +250,9 @@ def set_threads(n: int) -> None:
 # Finaliser, Algorithm 4.6: inverse transform of the grid
 # with the uv origin at pixel (N/2,N/2) (eq 2.8 :516, unnormalised, +j), divide by
 # the normaliser (eq 4.5), by the taper (eq 2.9 :523, reading 14) and by the sinc
-# of the nearest-sample lookup (eq 2.13 :561-564). Stokes conversion left out.
-# numpy's FFT is the library primitive; shifts put the origin where the paper does.
+# of the nearest-sample lookup (eq 2.13 :561-564). numpy's FFT is the library primitive;
+# shifts put the origin where the paper does. Step 2's Stokes conversion (:1660, :1668) is
+# finalize_stokes below (the paper prints no formulas: reading 21).
 # ----------------------------------------------------------------------------
 def transform_grid(grid):
     """img[pol][b][a] = sum_{Y,X} grid[Y][X][pol] e^{+j2pi((X-N/2)a+(Y-N/2)b)/N}, a,b in [-N/2,N/2)."""
@@ -270,6 +271,33 @@ def finalize(grid, norm, beta):
     img = transform_grid(grid).real
     with np.errstate(divide="ignore", invalid="ignore"):
         out = img / (np.asarray(norm)[:, None, None] * corr[None])
+    out[:, corr == 0.0] = 0.0
+    return out
+
+
+# Step 2 of Algorithm 4.6, "Convert to multiple-Stokes image and normalise".
+# The paper gives no formulas (reading 21): polarisations are taken as the linear-feed correlations
+# of a LOFAR MeasurementSet in its order (XX, XY, YX, YY), whose relation to the Stokes visibilities is
+# the textbook one, XX = I + Q, XY = U + jV, YX = U - jV, YY = I - Q; inverted per image pixel on the
+# NORMALISED complex images D_p = img_p / N_p ("convert ... and normalise"):
+#   4 pol: I = (D_XX + D_YY)/2, Q = (D_XX - D_YY)/2, U = (D_XY + D_YX)/2, V = (D_XY - D_YX)/(2j)
+#   2 pol (XX, YY): I, Q as above;   1 pol: I = D_0 (the only Stokes "that can be calculated", :1660).
+# The real part is taken after the combination (V needs the imaginary parts), then steps 3-4 as finalize.
+def finalize_stokes(grid, norm, beta):
+    n, npol = grid.shape[0], grid.shape[2]
+    a = np.arange(-n // 2, n // 2, dtype=np.float64)
+    psi = taper(2.0 * a / n)
+    snc = np.sinc(a / (n * beta))
+    corr = np.outer(psi * snc, psi * snc)
+    d = transform_grid(grid) / np.asarray(norm, dtype=np.float64)[:, None, None]
+    if npol == 4:
+        st = np.stack([(d[0] + d[3]) / 2, (d[0] - d[3]) / 2, (d[1] + d[2]) / 2, (d[1] - d[2]) / 2j])
+    elif npol == 2:
+        st = np.stack([(d[0] + d[1]) / 2, (d[0] - d[1]) / 2])
+    else:
+        st = d
+    with np.errstate(divide="ignore", invalid="ignore"):
+        out = st.real / corr[None]
     out[:, corr == 0.0] = 0.0
     return out
 

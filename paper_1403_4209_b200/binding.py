@@ -46,6 +46,7 @@ SIGNATURES = {
     "ig_measure_fp32_peak": (_i, [_vp, _vp, C.POINTER(_d)]),
     "ig_set_sort_tile_shift": (_i, [_vp, _i]),
     "ig_set_gather_min_support": (_i, [_vp, _i]),
+    "ig_set_stokes_output": (_i, [_vp, _i]),
     "ig_measure_commit_rate": (_i, [_vp, _vp, _sz, _i, C.POINTER(_d)]),
     "ig_get_timing": (_i, [_vp, _i, C.POINTER(C.c_float), C.POINTER(C.c_float)]),
     "ig_reset_accumulators": (_i, [_vp]),
@@ -258,6 +259,9 @@ class Gridder:
 
     def set_gather_min_support(self, s: int):
         self._check(self.lib.ig_set_gather_min_support(self.ctx, int(s)), "ig_set_gather_min_support")
+
+    def set_stokes_output(self, on: bool):
+        self._check(self.lib.ig_set_stokes_output(self.ctx, int(bool(on))), "ig_set_stokes_output")
 
     def set_sort_tile_shift(self, shift: int):
         self._check(self.lib.ig_set_sort_tile_shift(self.ctx, int(shift)), "ig_set_sort_tile_shift")

@@ -366,7 +366,7 @@ ig_status ig_finalize_channel(ig_ctx* c, int channel, float* image_dev, double* 
     if (!c || !image_dev || channel < 0 || channel >= IG_MAX_CHAN_GRIDS) return IG_EINVAL;
     if (!c->bound || !c->have_bank || !c->per_channel) return fail(c, IG_ESTATE, "per-channel grids are not in use");
     if ((size_t)(channel + 1) * ig_grid_bytes(c) > c->grid_bytes) return fail(c, IG_EINVAL, "no such channel grid");
-    int r = ig_run_finalize(c, channel, image_dev, norm_host);
+    int r = ig_run_finalize(c, channel, image_dev, norm_host, c->stokes);
     if (r == -2) return IG_ENOMEM;
     return r < 0 ? IG_ECUDA : IG_OK;
 }
@@ -375,9 +375,15 @@ ig_status ig_finalize(ig_ctx* c, float* image_dev, double* norm_host) {
     if (!c || !image_dev) return IG_EINVAL;
     if (!c->bound || !c->have_bank) return fail(c, IG_ESTATE, "nothing to finalise");
     if (c->per_channel) return fail(c, IG_ESTATE, "per-channel grids: use ig_finalize_channel");
-    int r = ig_run_finalize(c, -1, image_dev, norm_host);
+    int r = ig_run_finalize(c, -1, image_dev, norm_host, c->stokes);
     if (r == -2) return IG_ENOMEM;
     return r < 0 ? IG_ECUDA : IG_OK;
+}
+
+ig_status ig_set_stokes_output(ig_ctx* c, int on) {
+    if (!c) return IG_EINVAL;
+    c->stokes = on != 0;
+    return IG_OK;
 }
 
 ig_status ig_get_stats(ig_ctx* c, long long* g, long long* d, long long* u) {

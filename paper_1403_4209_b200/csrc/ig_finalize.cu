@@ -4,7 +4,9 @@
 // taper correction eq 2.9 (:523), sinc of the nearest-sample lookup eq 2.13 (:561-564).
 // Transform convention eq 2.8 (:516): img[b][a] = sum grid[Y][X] e^{+j 2 pi ((X-N/2)a + (Y-N/2)b)/N},
 // a,b in [-N/2, N/2), i.e. an unnormalised inverse DFT with both origins at index N/2.
-// Stokes conversion is not done (formulas absent from the paper).
+// Step 2's Stokes conversion (:1660, :1668; reading 21: linear feeds XX, XY, YX, YY) is ig_finalize_stokes:
+// the transform is linear, so the combination of the normalised polarisations is formed on the uv-grid
+// (k_fin_combine) and one inverse FFT per Stokes parameter follows.
 #include <cufft.h>
 #include <math.h>
 #include "ig_internal.h"
@@ -18,6 +20,26 @@ __global__ void k_fin_extract(const float2* __restrict__ grid, float2* __restric
     constexpr int PP = NPOL == 4 ? 2 : NPOL;
     const size_t base = NPOL == 4 ? (size_t)(pol >> 1) * N * N * 2 : 0;
     plane[(size_t)y * N + x] = grid[base + ((size_t)sy * N + sx) * PP + (NPOL == 4 ? (pol & 1) : pol)];
+}
+
+// plane = sum_p coef[p] * grid_p (complex coefficients): one Stokes parameter's uv-grid, normalisers folded into coef
+template <int NPOL>
+__global__ void k_fin_combine(const float2* __restrict__ grid, float2* __restrict__ plane, int N, float2 c0, float2 c1,
+                              float2 c2, float2 c3) {
+    int x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y;
+    if (x >= N) return;
+    int sx = (x + N / 2) % N, sy = (y + N / 2) % N;
+    const float2 cf[4] = {c0, c1, c2, c3};
+    constexpr int PP = NPOL == 4 ? 2 : NPOL;
+    float re = 0.f, im = 0.f;
+#pragma unroll
+    for (int pol = 0; pol < NPOL; ++pol) {
+        const size_t base = NPOL == 4 ? (size_t)(pol >> 1) * N * N * 2 : 0;
+        const float2 g = grid[base + ((size_t)sy * N + sx) * PP + (NPOL == 4 ? (pol & 1) : pol)];
+        re += cf[pol].x * g.x - cf[pol].y * g.y;
+        im += cf[pol].x * g.y + cf[pol].y * g.x;
+    }
+    plane[(size_t)y * N + x] = make_float2(re, im);
 }
 
 __global__ void k_fin_write(const float2* __restrict__ plane, float* __restrict__ image, const double* __restrict__ corr,
@@ -41,7 +63,7 @@ size_t ig_finalize_scratch_bytes(const ig_ctx* c) {
     return ig_align(N * N * 8) + ig_align(N * 8) + ig_align(fft_work_bytes((int)N));
 }
 
-int ig_run_finalize(ig_ctx* c, int channel, float* image, double* norm_host) {
+int ig_run_finalize(ig_ctx* c, int channel, float* image, double* norm_host, bool stokes) {
     const int N = c->prm.N, npol = c->prm.npol;
     if (c->work_bytes < ig_finalize_scratch_bytes(c)) { c->err = "work buffer too small for ig_finalize"; return -2; }
     IgAccum acc;
@@ -79,8 +101,28 @@ int ig_run_finalize(ig_ctx* c, int channel, float* image, double* norm_host) {
     cufftSetStream(plan, c->stream);
     int launches = 0;
     dim3 g((N + 255) / 256, N), b(256);
+    // Stokes parameter s = sum_p M[s][p] D_p with D_p = img_p / N_p (reading 21); the coefficients carry N_ref / N_p so that
+    // the grids keep their scale through the fp32 FFT and k_fin_write divides by N_ref = N_0 in fp64
+    const double nref = acc.norm[0];
     for (int q = 0; q < npol; ++q) {
-        switch (npol) {
+        if (stokes && npol > 1) {
+            double m[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};          // complex coefficient per polarisation
+            if (npol == 4) {
+                if (q == 0) { m[0][0] = 0.5; m[3][0] = 0.5; }            // I = (XX + YY)/2
+                if (q == 1) { m[0][0] = 0.5; m[3][0] = -0.5; }           // Q = (XX - YY)/2
+                if (q == 2) { m[1][0] = 0.5; m[2][0] = 0.5; }            // U = (XY + YX)/2
+                if (q == 3) { m[1][1] = -0.5; m[2][1] = 0.5; }           // V = (XY - YX)/(2j)
+            } else {
+                m[0][0] = 0.5; m[1][0] = q == 0 ? 0.5 : -0.5;            // (XX, YY): I, Q
+            }
+            float2 cf[4];
+            for (int p = 0; p < 4; ++p) {
+                const double sc = (p < npol && acc.norm[p] != 0.0) ? nref / acc.norm[p] : 0.0;
+                cf[p] = make_float2((float)(m[p][0] * sc), (float)(m[p][1] * sc));
+            }
+            if (npol == 4) k_fin_combine<4><<<g, b, 0, c->stream>>>(grid, plane, N, cf[0], cf[1], cf[2], cf[3]);
+            else k_fin_combine<2><<<g, b, 0, c->stream>>>(grid, plane, N, cf[0], cf[1], cf[2], cf[3]);
+        } else switch (npol) {
             case 1: k_fin_extract<1><<<g, b, 0, c->stream>>>(grid, plane, N, q); break;
             case 2: k_fin_extract<2><<<g, b, 0, c->stream>>>(grid, plane, N, q); break;
             default: k_fin_extract<4><<<g, b, 0, c->stream>>>(grid, plane, N, q); break;
@@ -88,7 +130,7 @@ int ig_run_finalize(ig_ctx* c, int channel, float* image, double* norm_host) {
         if (cufftExecC2C(plan, (cufftComplex*)plane, (cufftComplex*)plane, CUFFT_INVERSE) != CUFFT_SUCCESS) {
             cufftDestroy(plan); c->err = "cufftExecC2C failed"; return -1;
         }
-        k_fin_write<<<g, b, 0, c->stream>>>(plane, image + (size_t)q * N * N, d_corr, N, acc.norm[q]);
+        k_fin_write<<<g, b, 0, c->stream>>>(plane, image + (size_t)q * N * N, d_corr, N, (stokes && npol > 1) ? nref : acc.norm[q]);
         launches += 3;
     }
     cudaError_t e = cudaStreamSynchronize(c->stream);

@@ -70,6 +70,7 @@ struct ig_ctx {
     int tile_shift = 0;                       // ig_set_sort_tile_shift (0 = automatic: N/8 cells, at least 128)
     int gather_min = IG_GATHER_MIN_DEFAULT;   // ig_set_gather_min_support
     bool count_commits = false;               // ig_set_commit_counting
+    bool stokes = false;                      // ig_set_stokes_output: the finaliser writes I,Q,U,V instead of the correlations
     // bank description (host copies)
     std::vector<int> support;
     std::vector<uint32_t> koff;
@@ -110,7 +111,7 @@ int ig_launch_bank(ig_ctx* c, char* scratch, size_t scratch_bytes);
 size_t ig_bank_scratch_bytes(const ig_ctx* c);
 int ig_launch_zeta(ig_ctx* c);
 int ig_detect_supports(ig_ctx* c, char* scratch, size_t scratch_bytes, int* table);
-int ig_run_finalize(ig_ctx* c, int channel, float* image, double* norm_host);   // channel < 0: the single grid
+int ig_run_finalize(ig_ctx* c, int channel, float* image, double* norm_host, bool stokes);   // channel < 0: the single grid
 size_t ig_finalize_scratch_bytes(const ig_ctx* c);
 
 #define IG_CUDA_OK(ctx, call)                                                        \

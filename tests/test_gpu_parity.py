@@ -652,3 +652,46 @@ def test_point_source_end_to_end(orc, torch_cuda):
             inner = slice(n // 8, n - n // 8)
             assert np.abs(img - want)[inner, inner].max() < 2e-4
     assert amp["wproj"] > 0.97 and amp["plain"] < 0.6, amp
+
+
+@pytest.mark.parametrize("npol", [4, 2, 1])
+def test_stokes_output_matches_oracle(npol, orc, torch_cuda):
+    """ig_set_stokes_output: step 2 of Algorithm 4.6 (reading 21) on the device against the oracle's
+    finalize_stokes on the oracle's grid of the same polarised point source plus noise; the source's Stokes parameters
+    come back at its pixel."""
+    from paper_1403_4209_b200.binding import Gridder
+    C = 299792458.0
+    rng = np.random.default_rng(41 + npol)
+    n, du, beta, S, nrec = 128, 20.0, 8, 7, 5000
+    umax = 0.4 * n * du
+    u, v = rng.uniform(-umax, umax, nrec), rng.uniform(-umax, umax, nrec)
+    a0, b0 = -21, 13
+    I, Q, U, V = 1.0, -0.25, 0.2, 0.1
+    ph = np.exp(-2j * np.pi * (u * a0 + v * b0) / (n * du))
+    corr = {4: [I + Q, U + 1j * V, U - 1j * V, I - Q], 2: [I + Q, I - Q], 1: [I]}[npol]
+    vis = np.stack([c * ph for c in corr], axis=-1).reshape(nrec, 1, npol)
+    vis = (vis + 0.05 * (rng.standard_normal(vis.shape) + 1j * rng.standard_normal(vis.shape))).astype(np.complex64)
+    wt = (np.array([1.0, 0.5, 0.8, 0.6])[:npol] * np.ones((nrec, 1, 1))).astype(np.float32)
+    uvw = np.ascontiguousarray(np.column_stack([u, v, np.zeros(nrec)]))
+    bl = (np.arange(nrec) % 31).astype(np.int32)
+    sup = np.array([S], dtype=np.int32)
+    bank, off = orc.build_bank(sup, 0.0, du, beta, S)
+    idx = orc.index_records(uvw, [C], n, 1 / (n * du), beta, 1, 0.0, sup)
+    gr, nrm, _ = orc.grid_records(idx, vis, wt, n, beta, sup, bank, off)
+    want = orc.finalize_stokes(gr, nrm, beta)
+    g = Gridder(n, 1 / (n * du), 1, beta, S, npol)
+    g.allocate(sup)
+    g.debug_set_wkernels(0.0, bank.astype(np.complex64))
+    d = "cuda:0"
+    g.grid_visibilities(torch_cuda.from_numpy(uvw).to(d), torch_cuda.from_numpy(bl).to(d), np.array([C]),
+                        torch_cuda.from_numpy(vis).to(d), torch_cuda.from_numpy(wt).to(d))
+    plain, _ = g.finalize()
+    g.set_stokes_output(True)
+    img, norm = g.finalize()
+    got = img.cpu().numpy().astype(np.float64)
+    assert got.shape == want.shape
+    inner = slice(n // 8, n - n // 8)
+    assert np.abs(got - want)[:, inner, inner].max() <= 2e-4 * np.abs(want[:, inner, inner]).max()
+    assert np.abs(got[:, b0 + n // 2, a0 + n // 2] - [I, Q, U, V][:npol]).max() < 2e-2
+    if npol > 1:        # the switch changed the output: the plain images are the correlations
+        assert np.abs(plain.cpu().numpy()[0, b0 + n // 2, a0 + n // 2] - (I + Q)) < 2e-2
