@@ -316,6 +316,9 @@ def bench_config(args, config, dev, ranks, steps, warmup, want_e2e, fp32_peak, c
     split = [g.timing(k) for k in range(min(steps, 64))]
     ingest_ms = float(np.mean([s[0] for s in split]))
     gridder_ms = float(np.mean([s[1] for s in split]))
+    gsplit = [g.gridder_split(k) for k in range(min(steps, 64))]
+    window_ms = float(np.mean([s[0] for s in gsplit]))
+    gather_ms = float(np.mean([s[1] for s in gsplit]))
     ms_step = ms_total / steps
 
     # end to end: host buffers through ig_grid_host, H2D copies and the D2H read of the step's result inside
@@ -348,6 +351,7 @@ def bench_config(args, config, dev, ranks, steps, warmup, want_e2e, fp32_peak, c
         "workload": WORKLOADS[config - 1], "ms_per_step": ms_step, "ingest_ms": ingest_ms, "gridder_ms": gridder_ms,
         "updates_per_s": world * updates / (ms_step * 1e-3), "visibilities_per_s": world * gridded / (ms_step * 1e-3),
         "gridder_updates_per_s": updates / (gridder_ms * 1e-3),
+        "gridder_window_ms": window_ms, "gridder_gather_ms": gather_ms,
         "records_gridded": gridded, "records_dropped": dropped, "updates_per_step": updates,
         "records_compressed": compressed, "launches_per_step": launches_per_step, "steps": steps, "warmup": warmup,
         "roofline": roof,
@@ -396,7 +400,7 @@ def run_ours(args):
                 continue
             r = bench_config(args, c, dev, ranks, max(3, min(args.steps, 10)), max(3, min(args.warmup, 5)), False, fp32_peak,
                              commit_rate_l2, True)
-            per_config[WORKLOADS[c - 1]] = {k: r[k] for k in ("ms_per_step", "ingest_ms", "gridder_ms", "updates_per_s", "visibilities_per_s",
+            per_config[WORKLOADS[c - 1]] = {k: r[k] for k in ("ms_per_step", "ingest_ms", "gridder_ms", "gridder_window_ms", "gridder_gather_ms", "updates_per_s", "visibilities_per_s",
                                                               "updates_per_step", "records_gridded", "steps", "warmup", "clocks")}
             per_config[WORKLOADS[c - 1]]["roofline"] = {k: r["roofline"][k] for k in ("bound", "frac", "frac_alu", "frac_hbm_model", "t_flop_ms",
                                                                                      "t_byte_ms", "commits", "commits_measured")}
@@ -432,6 +436,7 @@ def run_ours(args):
                         "note": "value counts every gridded record (thesis total rate, PAPER.md:1767); "
                                 "real rate = value * (1 - records_compressed / records_gridded)"},
         "ingest_ms": main["ingest_ms"], "gridder_ms": main["gridder_ms"], "gridder_updates_per_s": main["gridder_updates_per_s"],
+        "gridder_window_ms": main["gridder_window_ms"], "gridder_gather_ms": main["gridder_gather_ms"],
         "roofline": main["roofline"], "ingest": main["ingest"], "cpu_baseline": cpu, "e2e": main["e2e"],
         "gpu_launches": main["launches_per_step"] * args.steps,
         "clocks": main["clocks"], "setup": main["setup"], "per_config": per_config,

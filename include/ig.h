@@ -151,7 +151,7 @@ ig_status ig_set_stokes_output(ig_ctx* ctx, int on);
 /* Step C runs two work distributions: records with support < s keep Romein's moving window
  * (registers follow a track, atomics when a pixel leaves the window, :710-742); records with support >= s go to
  * the fixed-tile gather gridder (a warp owns an 8 x 16 pixel tile in registers, records binned by tile, no atomics
- * in the loop). Default 17. s = 1: everything through the gather gridder; s > IG_MAX_SUPPORT: nothing. Same grid
+ * in the loop). Default 25 (measured crossover on configurations 3-5). s = 1: everything through the gather gridder; s > IG_MAX_SUPPORT: nothing. Same grid
  * up to fp32 summation order. Per-channel grids always use the moving window. */
 ig_status ig_set_gather_min_support(ig_ctx* ctx, int s);
 
@@ -194,6 +194,9 @@ ig_status ig_measure_commit_rate(void* cuda_stream, void* buf_dev, size_t bytes,
  * stream): ingest (A1-A3) and gridder (C). calls_back = 0 is the last non-empty call, 1 the one
  * before, ... up to 63. Waits for that call to finish. */
 ig_status ig_get_timing(ig_ctx* ctx, int calls_back, float* ingest_ms, float* gridder_ms);
+/* The gridder time of that call split into its two work distributions: the moving-window kernel and the
+ * fixed-tile gather phase (plan + scatter + gather kernel; 0 when no support reaches ig_set_gather_min_support). */
+ig_status ig_get_gridder_split(ig_ctx* ctx, int calls_back, float* window_ms, float* gather_ms);
 /* Zero the normaliser and the statistics (for a caller that zeroes the grid to start a new
  * image with the same bank). Asynchronous. */
 ig_status ig_reset_accumulators(ig_ctx* ctx);

@@ -49,6 +49,7 @@ SIGNATURES = {
     "ig_set_stokes_output": (_i, [_vp, _i]),
     "ig_measure_commit_rate": (_i, [_vp, _vp, _sz, _i, C.POINTER(_d)]),
     "ig_get_timing": (_i, [_vp, _i, C.POINTER(C.c_float), C.POINTER(C.c_float)]),
+    "ig_get_gridder_split": (_i, [_vp, _i, C.POINTER(C.c_float), C.POINTER(C.c_float)]),
     "ig_reset_accumulators": (_i, [_vp]),
     "ig_last_launches": (_i, [_vp]),
     "ig_debug_indices": (_i, [_vp, _vp, _ll, _vp, _i, _vp, _vp, _vp, _vp, _vp, _vp]),
@@ -300,6 +301,12 @@ class Gridder:
         """(ingest_ms, gridder_ms) of the ig_grid call `calls_back` calls ago."""
         a, b = C.c_float(), C.c_float()
         self._check(self.lib.ig_get_timing(self.ctx, calls_back, C.byref(a), C.byref(b)), "ig_get_timing")
+        return a.value, b.value
+
+    def gridder_split(self, calls_back=0):
+        """(moving-window ms, gather-phase ms) of the gridder time of that ig_grid call."""
+        a, b = C.c_float(), C.c_float()
+        self._check(self.lib.ig_get_gridder_split(self.ctx, calls_back, C.byref(a), C.byref(b)), "ig_get_gridder_split")
         return a.value, b.value
 
     def reset(self):

@@ -63,7 +63,7 @@ int install_table(ig_ctx* c, const int* table) {
     c->bank_elems = e;
     if (bank_head_bytes(c) + e * 8 > c->bank_bytes) { c->err = "bank buffer too small (see ig_bank_bytes)"; return -2; }
     std::vector<IgPlaneEntry> pe(P);
-    for (int p = 0; p < P; ++p) { pe[p].support = table[p]; pe[p].koff = c->koff[p]; }
+    for (int p = 0; p < P; ++p) { pe[p].support = table[p]; pe[p].koff = c->koff[p]; pe[p].magic = (uint32_t)((1ull << 32) / (unsigned)table[p]) + 1u; pe[p].pad_ = 0u; }
     IG_CUDA_OK(c, cudaMemcpyAsync(c->d_planes, pe.data(), (size_t)P * sizeof(IgPlaneEntry), cudaMemcpyHostToDevice, c->stream));
     IG_CUDA_OK(c, cudaStreamSynchronize(c->stream));
     return 0;
@@ -87,6 +87,8 @@ ig_status ig_create(ig_ctx** out, int grid_n, double cell_rad, int n_wplanes, in
     if (!c) return IG_ENOMEM;
     c->prm.N = grid_n; c->prm.beta = oversampling; c->prm.P = n_wplanes; c->prm.npol = n_pol;
     c->prm.shift = (oversampling + 1) / 2 - 1;
+    c->prm.bshift = -1;
+    for (int b = 0; b < 5; ++b) if (oversampling == (1 << b)) c->prm.bshift = b;
     c->cell_rad = cell_rad;
     c->du = 1.0 / ((double)grid_n * cell_rad);
     c->prm.ku = (double)oversampling / (IG_C_M_S * c->du);
@@ -99,6 +101,7 @@ ig_status ig_create(ig_ctx** out, int grid_n, double cell_rad, int n_wplanes, in
 void ig_destroy(ig_ctx* c) {
     if (!c) return;
     for (auto& t : c->ev) for (auto& e : t) if (e) cudaEventDestroy(e);
+
     for (auto& e : c->ev_copied) if (e) cudaEventDestroy(e);
     for (auto& e : c->ev_free) if (e) cudaEventDestroy(e);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
@@ -155,6 +158,7 @@ ig_status ig_bind(ig_ctx* c, void* grid_dev, size_t grid_bytes, void* work_dev, 
     for (auto& t : c->ev)
         for (auto& ev : t)
             if (!ev && cudaEventCreate(&ev) != cudaSuccess) return fail(c, IG_ECUDA, "cudaEventCreate failed");
+
     c->bound = true;
     return IG_OK;
 }
@@ -259,6 +263,7 @@ ig_status ig_grid(ig_ctx* c, const double* uvw, const int* baseline_id, long lon
     n = ig_launch_gridder(c, records, smax, L.nrb, nchan);
     if (n < 0) return IG_ECUDA;
     c->launches += n;
+    cudaEventRecord(ev[2], c->stream);
     bool any_gather = false;
     for (int p = 0; p < c->prm.P; ++p) any_gather |= c->support[p] >= gather_min;
     if (any_gather) {
@@ -268,7 +273,7 @@ ig_status ig_grid(ig_ctx* c, const double* uvw, const int* baseline_id, long lon
         if (n < 0) return IG_ECUDA;
         c->launches += n;
     }
-    cudaEventRecord(ev[2], c->stream);
+    cudaEventRecord(ev[3], c->stream);
     c->n_timed += 1;
     return IG_OK;
 }
@@ -437,12 +442,25 @@ ig_status ig_get_timing(ig_ctx* c, int calls_back, float* ingest_ms, float* grid
     if (!c || calls_back < 0 || calls_back >= IG_TIMING_RING) return IG_EINVAL;
     if (c->n_timed <= calls_back) return fail(c, IG_ESTATE, "no such timed ig_grid call");
     cudaEvent_t* ev = c->ev[(c->n_timed - 1 - calls_back) % IG_TIMING_RING];
-    if (cudaEventSynchronize(ev[2]) != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_get_timing: ") + cudaGetErrorString(cudaGetLastError()));
+    if (cudaEventSynchronize(ev[3]) != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_get_timing: ") + cudaGetErrorString(cudaGetLastError()));
     float a = 0, b = 0;
     cudaEventElapsedTime(&a, ev[0], ev[1]);
-    cudaEventElapsedTime(&b, ev[1], ev[2]);
+    cudaEventElapsedTime(&b, ev[1], ev[3]);
     if (ingest_ms) *ingest_ms = a;
     if (gridder_ms) *gridder_ms = b;
+    return IG_OK;
+}
+
+ig_status ig_get_gridder_split(ig_ctx* c, int calls_back, float* window_ms, float* gather_ms) {
+    if (!c || calls_back < 0 || calls_back >= IG_TIMING_RING) return IG_EINVAL;
+    if (c->n_timed <= calls_back) return fail(c, IG_ESTATE, "no such timed ig_grid call");
+    cudaEvent_t* ev = c->ev[(c->n_timed - 1 - calls_back) % IG_TIMING_RING];
+    if (cudaEventSynchronize(ev[3]) != cudaSuccess) return fail(c, IG_ECUDA, std::string("ig_get_gridder_split: ") + cudaGetErrorString(cudaGetLastError()));
+    float a = 0, b = 0;
+    cudaEventElapsedTime(&a, ev[1], ev[2]);
+    cudaEventElapsedTime(&b, ev[2], ev[3]);
+    if (window_ms) *window_ms = a;
+    if (gather_ms) *gather_ms = b;
     return IG_OK;
 }
 

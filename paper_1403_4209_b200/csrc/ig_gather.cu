@@ -31,9 +31,19 @@
 #define IG_GT 32          // origin tile side in pixels
 #define IG_GT_SHIFT 5
 #define IG_GCH 256        // records per gather item
+#ifndef IG_GW
 #define IG_GW 8           // warps per gather CTA
+#endif
 #define IG_GR 4           // pixel row groups per lane: sub-tile = 8 wide x 4*IG_GR tall
+#ifndef IG_XP
+#define IG_XP 0          // timing experiments only (results are wrong when non-zero)
+#endif
+#ifndef IG_GPIPE
+#define IG_GPIPE 1       // two records in flight per warp
+#endif
+#ifndef IG_GCTAS_PER_SM
 #define IG_GCTAS_PER_SM 3
+#endif
 
 __device__ __forceinline__ uint32_t g_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ uint32_t g_lanemask_lt() {
@@ -148,63 +158,108 @@ __global__ void __launch_bounds__(256) k_gather_scatter(const char* __restrict__
 }
 
 // ---------------------------------------------------------------------------------------------------------
-typedef unsigned long long gf32x2;
-__device__ __forceinline__ void g_unpack2(gf32x2 v, float& lo, float& hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+// One record against one sub-tile (8 columns x 16 rows = 4 row groups of 4 rows, one pixel per lane and row group),
+// in two steps so that the kernel values of the NEXT record are in flight while the current one is accumulated
+// (a warp's loads are otherwise strictly serial: header -> addresses -> values -> FMAs).
+//   g_prepare  header {ox, oy, S, kbase} (footprint origin relative to the origin tile, support, first element of the
+//              record's S x S matrix) is a shared-memory broadcast; the lane's tap is (ty0 + 4k, tx) and lies in the
+//              footprint iff both are in [0, S); the four kernel values are requested with predicated read-only
+//              loads (zero outside the footprint).
+//   g_apply    the footprint's rows reach a contiguous range [KA, KB] of the row groups (warp-uniform);
+//              g_groups<KA, KB> is the straight-line code for that range: per row group and polarisation
+//                acc += (v_re, v_re) * (k_re, k_im);   acc += (-v_im, v_im) * (k_im, k_re)     (two packed FMAs, FFMA2)
+//              Row groups outside the range cost nothing, so the lanes wasted in y are at most 3 rows per record.
+struct GHit {
+    const char* ep;      // the entry in shared memory
+    int S, oy;           // support; footprint's first row relative to the sub-tile
+    float2 kv[IG_GR];
+};
 
-// One row group (4 rows of the sub-tile, one pixel per lane) of one record, as ONE PTX block so that the sums stay in
-// place and no branch is needed: p = this lane's pixel lies inside the footprint (ty = ty0 + 4K in [0, S); lanes
-// outside the footprint's columns carry ty0 = 2^30); the kernel value is a predicated read-only load and ZERO outside
-// the footprint, so the FMAs run unpredicated (FFMA2 has no predicated form: ptxas turns "@p fma.f32x2" into FFMA2 + 2 SEL);
-// per polarisation acc += (v_re,v_re)*(k_re,k_im); acc += (-v_im,v_im)*(k_im,k_re)   (two packed FMAs, SASS FFMA2).
-template <int K>
-__device__ __forceinline__ void g_rowgroup(gf32x2 (&acc)[4], const gf32x2 (&vre)[4], const gf32x2 (&vim)[4], int ty0, int S,
-                                           const unsigned long long* base, unsigned stride_bytes) {
-    asm volatile("{\n\t.reg .pred p;\n\t.reg .b64 kv, ks, ad;\n\t.reg .f32 kr, ki;\n\t.reg .s32 t;\n\t"
-                 "add.s32 t, %4, %8;\n\t"
-                 "setp.lt.u32 p, t, %5;\n\t"
-                 "mad.wide.u32 ad, %6, %9, %7;\n\t"
-                 "mov.b64 kv, 0;\n\t@p ld.global.nc.b64 kv, [ad];\n\t"
-                 "mov.b64 {kr, ki}, kv;\n\t"
-                 "mov.b64 ks, {ki, kr};\n\t"
-                 "fma.rn.f32x2 %0, %10, kv, %0;\n\tfma.rn.f32x2 %1, %12, kv, %1;\n\t"
-                 "fma.rn.f32x2 %2, %14, kv, %2;\n\tfma.rn.f32x2 %3, %16, kv, %3;\n\t"
-                 "fma.rn.f32x2 %0, %11, ks, %0;\n\tfma.rn.f32x2 %1, %13, ks, %1;\n\t"
-                 "fma.rn.f32x2 %2, %15, ks, %2;\n\tfma.rn.f32x2 %3, %17, ks, %3;\n\t}"
-                 : "+l"(acc[0]), "+l"(acc[1]), "+l"(acc[2]), "+l"(acc[3])
-                 : "r"(ty0), "r"(S), "r"(stride_bytes), "l"(base), "n"(4 * K), "n"(K),
-                   "l"(vre[0]), "l"(vim[0]), "l"(vre[1]), "l"(vim[1]), "l"(vre[2]), "l"(vim[2]), "l"(vre[3]), "l"(vim[3]));
+__device__ __forceinline__ void g_prepare(GHit& H, const char* __restrict__ ep, int sub_x, int sub_y, int lx, int lr,
+                                          const float2* __restrict__ bank) {
+    const int4 h = *reinterpret_cast<const int4*>(ep);              // warp-wide broadcast
+    H.ep = ep;
+    H.S = h.z;
+    H.oy = h.y - sub_y;
+    const int tx = lx - (h.x - sub_x);
+    const int ty0 = lr - H.oy;
+    const bool col_in = (unsigned)tx < (unsigned)h.z;
+    const uint32_t e0 = (uint32_t)h.w + (uint32_t)(ty0 * h.z + tx);  // element index of tap (ty0, tx); wraps harmlessly when unused
+#pragma unroll
+    for (int k = 0; k < IG_GR; ++k) {
+        H.kv[k] = make_float2(0.f, 0.f);
+#if IG_XP == 1   /* experiment: no kernel loads */
+        if (col_in && (unsigned)(ty0 + 4 * k) < (unsigned)h.z) H.kv[k] = make_float2(__uint_as_float(e0 + 4 * k * h.z), 1.f);
+#else
+        if (col_in && (unsigned)(ty0 + 4 * k) < (unsigned)h.z) H.kv[k] = __ldg(bank + (e0 + (uint32_t)(4 * k * h.z)));
+#endif
+    }
 }
-template <int K>
-__device__ __forceinline__ void g_rowgroup(gf32x2 (&acc)[2], const gf32x2 (&vre)[2], const gf32x2 (&vim)[2], int ty0, int S,
-                                           const unsigned long long* base, unsigned stride_bytes) {
-    asm volatile("{\n\t.reg .pred p;\n\t.reg .b64 kv, ks, ad;\n\t.reg .f32 kr, ki;\n\t.reg .s32 t;\n\t"
-                 "add.s32 t, %2, %6;\n\t"
-                 "setp.lt.u32 p, t, %3;\n\t"
-                 "mad.wide.u32 ad, %4, %7, %5;\n\t"
-                 "mov.b64 kv, 0;\n\t@p ld.global.nc.b64 kv, [ad];\n\t"
-                 "mov.b64 {kr, ki}, kv;\n\t"
-                 "mov.b64 ks, {ki, kr};\n\t"
-                 "fma.rn.f32x2 %0, %8, kv, %0;\n\tfma.rn.f32x2 %1, %10, kv, %1;\n\t"
-                 "fma.rn.f32x2 %0, %9, ks, %0;\n\tfma.rn.f32x2 %1, %11, ks, %1;\n\t}"
-                 : "+l"(acc[0]), "+l"(acc[1])
-                 : "r"(ty0), "r"(S), "r"(stride_bytes), "l"(base), "n"(4 * K), "n"(K),
-                   "l"(vre[0]), "l"(vim[0]), "l"(vre[1]), "l"(vim[1]));
+
+template <int NPOL, int KA, int KB>
+__device__ __forceinline__ void g_groups(float2 (&acc)[IG_GR][NPOL], const GHit& H) {
+    float2 vre[NPOL], vim[NPOL];
+#pragma unroll
+    for (int q = 0; q < NPOL; ++q) {
+        const float4 t = *reinterpret_cast<const float4*>(H.ep + 16 + 16 * q);   // {v_re, v_re, -v_im, v_im}
+        vre[q] = make_float2(t.x, t.y);
+        vim[q] = make_float2(t.z, t.w);
+    }
+#pragma unroll
+    for (int k = KA; k <= KB; ++k) {
+        const float2 ks = make_float2(H.kv[k].y, H.kv[k].x);
+#if IG_XP == 2   /* experiment: one FMA per kernel value */
+        acc[k][0] = __ffma2_rn(vre[0], H.kv[k], acc[k][0]);
+        (void)ks; (void)vim;
+#else
+#pragma unroll
+        for (int q = 0; q < NPOL; ++q) {
+            acc[k][q] = __ffma2_rn(vre[q], H.kv[k], acc[k][q]);
+            acc[k][q] = __ffma2_rn(vim[q], ks, acc[k][q]);
+        }
+#endif
+    }
 }
-template <int K>
-__device__ __forceinline__ void g_rowgroup(gf32x2 (&acc)[1], const gf32x2 (&vre)[1], const gf32x2 (&vim)[1], int ty0, int S,
-                                           const unsigned long long* base, unsigned stride_bytes) {
-    asm volatile("{\n\t.reg .pred p;\n\t.reg .b64 kv, ks, ad;\n\t.reg .f32 kr, ki;\n\t.reg .s32 t;\n\t"
-                 "add.s32 t, %1, %5;\n\t"
-                 "setp.lt.u32 p, t, %2;\n\t"
-                 "mad.wide.u32 ad, %3, %6, %4;\n\t"
-                 "mov.b64 kv, 0;\n\t@p ld.global.nc.b64 kv, [ad];\n\t"
-                 "mov.b64 {kr, ki}, kv;\n\t"
-                 "mov.b64 ks, {ki, kr};\n\t"
-                 "fma.rn.f32x2 %0, %7, kv, %0;\n\t"
-                 "fma.rn.f32x2 %0, %8, ks, %0;\n\t}"
-                 : "+l"(acc[0])
-                 : "r"(ty0), "r"(S), "r"(stride_bytes), "l"(base), "n"(4 * K), "n"(K), "l"(vre[0]), "l"(vim[0]));
+
+template <int NPOL>
+__device__ __forceinline__ void g_apply(float2 (&acc)[IG_GR][NPOL], const GHit& H) {
+    const int ka = max(H.oy, 0) >> 2, kb = min(H.oy + H.S - 1, 4 * IG_GR - 1) >> 2;   // the record touches the sub-tile: 0 <= ka <= kb <= 3
+    switch (ka * 4 + kb) {
+#define IG_GCASE(A, B) case A * 4 + B: g_groups<NPOL, A, B>(acc, H); break;
+        IG_GCASE(0, 0) IG_GCASE(0, 1) IG_GCASE(0, 2) IG_GCASE(0, 3) IG_GCASE(1, 1) IG_GCASE(1, 2) IG_GCASE(1, 3)
+        IG_GCASE(2, 2) IG_GCASE(2, 3) IG_GCASE(3, 3)
+#undef IG_GCASE
+        default: break;
+    }
 }
+
+// Iterator over the records of the staged item that touch a sub-tile: ballots over groups of 32 staged headers.
+struct GScan {
+    const char* buf;
+    int count, g0, sub_x, sub_y, lane, gstride;
+    uint32_t m;
+    __device__ __forceinline__ void start(const char* b, int n, int sx, int sy, int ln, int gs) {
+        buf = b; count = n; sub_x = sx; sub_y = sy; lane = ln; gstride = gs; g0 = -32; m = 0u;
+    }
+    // next touching record (its entry), or nullptr when the item is exhausted; warp-uniform
+    __device__ __forceinline__ const char* next() {
+        while (m == 0u) {
+            g0 += 32;
+            if (g0 >= count) return nullptr;
+            bool hit = false;
+            if (g0 + lane < count) {
+                // footprint [ox, ox+S) x [oy, oy+S) against the sub-tile [sub_x, sub_x+8) x [sub_y, sub_y+16)
+                const int4 w = *reinterpret_cast<const int4*>(buf + (g0 + lane) * gstride);
+                const int ox = w.x - sub_x, oy = w.y - sub_y;
+                hit = ox < 8 && ox + w.z > 0 && oy < 4 * IG_GR && oy + w.z > 0;
+            }
+            m = __ballot_sync(0xffffffffu, hit);
+        }
+        const int b = __ffs(m) - 1;
+        m &= m - 1;
+        return buf + (g0 + b) * gstride;
+    }
+};
 
 template <int NPOL, bool COUNT>
 __global__ void __launch_bounds__(IG_GW * 32, IG_GCTAS_PER_SM)
@@ -219,7 +274,6 @@ k_gather(const char* __restrict__ entries, const uint4* __restrict__ items, cons
     const int lx = lane & 7, lr = lane >> 3;
     const unsigned n_items = plan_hdr[0];
     const unsigned long long plane_bytes = (unsigned long long)N * N * 16;   // 4 pol: two planes of pol pairs
-    const unsigned long long* __restrict__ bank64 = reinterpret_cast<const unsigned long long*>(bank);
     if (threadIdx.x == 0) {
         asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(g_smem_u32(&bar)), "r"(1) : "memory");
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -263,57 +317,52 @@ k_gather(const char* __restrict__ entries, const uint4* __restrict__ items, cons
             if (st >= nsub) break;
             const int sy = (int)st / nsx, sx = (int)st - sy * nsx;
             const int sub_x = sx * 8, sub_y = sy * (4 * IG_GR);        // sub-tile origin relative to the origin tile
-            gf32x2 acc[IG_GR][NPOL];
+            float2 acc[IG_GR][NPOL];
 #pragma unroll
             for (int k = 0; k < IG_GR; ++k)
 #pragma unroll
-                for (int q = 0; q < NPOL; ++q) acc[k][q] = 0ull;
-            for (int g0 = 0; g0 < count; g0 += 32) {
-                // which of these 32 records touch the sub-tile: footprint [ox, ox+S) x [oy, oy+S) against [sub_x, sub_x+8) x [sub_y, sub_y+16)
-                bool hit = false;
-                if (g0 + lane < count) {
-                    const int4 w = *reinterpret_cast<const int4*>(buf + (g0 + lane) * GSTRIDE);
-                    const int ox = w.x - sub_x, oy = w.y - sub_y;
-                    hit = ox < 8 && ox + w.z > 0 && oy < 4 * IG_GR && oy + w.z > 0;
-                }
-                uint32_t m = __ballot_sync(0xffffffffu, hit);
-                while (m) {
-                    const int b = __ffs(m) - 1;
-                    m &= m - 1;
-                    const char* ep = buf + (g0 + b) * GSTRIDE;
-                    const int4 h = *reinterpret_cast<const int4*>(ep);              // warp-wide broadcast: {ox, oy, S, kbase}
-                    gf32x2 vre[NPOL], vim[NPOL];
-#pragma unroll
-                    for (int q = 0; q < NPOL; ++q) {
-                        const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(ep + 16 + 16 * q);
-                        vre[q] = t.x; vim[q] = t.y;
-                    }
-                    const int S = h.z;
-                    const int tx = lx - (h.x - sub_x);                               // this lane's tap column
-                    const int ty = lr - (h.y - sub_y);                               // tap row of row group 0
-                    const int ty0 = (unsigned)tx < (unsigned)S ? ty : (1 << 30);     // columns outside the footprint never pass
-                    const unsigned long long* base = bank64 + (long long)(uint32_t)h.w + (long long)(ty * S + tx);
-                    const unsigned stride = 32u * (unsigned)S;                        // 4 rows of S taps of 8 bytes
-                    g_rowgroup<0>(acc[0], vre, vim, ty0, S, base, stride);
-                    g_rowgroup<1>(acc[1], vre, vim, ty0, S, base, stride);
-                    g_rowgroup<2>(acc[2], vre, vim, ty0, S, base, stride);
-                    g_rowgroup<3>(acc[3], vre, vim, ty0, S, base, stride);
+                for (int q = 0; q < NPOL; ++q) acc[k][q] = make_float2(0.f, 0.f);
+            GScan scan;
+            scan.start(buf, count, sub_x, sub_y, lane, GSTRIDE);
+            GHit ha, hb;
+            const char* e = scan.next();
+#if !IG_GPIPE
+            (void)hb;
+            while (e) {
+                g_prepare(ha, e, sub_x, sub_y, lx, lr, bank);
+                g_apply<NPOL>(acc, ha);
+                e = scan.next();
+            }
+#else
+            // two records in flight: the next one's kernel values are requested before the current one's FMAs
+            if (e) {
+                g_prepare(ha, e, sub_x, sub_y, lx, lr, bank);
+                for (;;) {
+                    e = scan.next();
+                    if (!e) { g_apply<NPOL>(acc, ha); break; }
+                    g_prepare(hb, e, sub_x, sub_y, lx, lr, bank);
+                    g_apply<NPOL>(acc, ha);
+                    e = scan.next();
+                    if (!e) { g_apply<NPOL>(acc, hb); break; }
+                    g_prepare(ha, e, sub_x, sub_y, lx, lr, bank);
+                    g_apply<NPOL>(acc, hb);
                 }
             }
+#endif
             // write the sub-tile: one vector reduction per touched pixel and polarisation pair (other items, and the
             // moving-window gridder, add to the same grid)
             const int x = (tile_x << IG_GT_SHIFT) + sub_x + lx;
 #pragma unroll
             for (int k = 0; k < IG_GR; ++k) {
                 const int y = (tile_y << IG_GT_SHIFT) + sub_y + 4 * k + lr;
-                gf32x2 any = 0ull;
+                uint32_t any = 0u;
 #pragma unroll
-                for (int q = 0; q < NPOL; ++q) any |= acc[k][q];
-                if (any != 0ull && x < N && y < N) {
+                for (int q = 0; q < NPOL; ++q) any |= __float_as_uint(acc[k][q].x) | __float_as_uint(acc[k][q].y);
+                if ((any << 1) != 0u && x < N && y < N) {          // some sum is not +-0
                     const size_t pix = (size_t)y * N + x;
                     float a[2 * NPOL];
 #pragma unroll
-                    for (int q = 0; q < NPOL; ++q) g_unpack2(acc[k][q], a[2 * q], a[2 * q + 1]);
+                    for (int q = 0; q < NPOL; ++q) { a[2 * q] = acc[k][q].x; a[2 * q + 1] = acc[k][q].y; }
                     if constexpr (NPOL == 1) {
                         asm volatile("red.global.add.v2.f32 [%0], {%1,%2};" ::"l"(grid + pix * 2), "f"(a[0]), "f"(a[1]) : "memory");
                     } else {
@@ -346,22 +395,23 @@ size_t ig_gather_max_items(const ig_ctx* c, long long n_chunks) {
 
 int ig_launch_gather(ig_ctx* c, const char* records, const uint32_t* gcount, long long n_chunks, uint32_t* tile_count,
                      uint32_t* tile_off, uint32_t* tile_cur, uint4* items, uint32_t* plan_hdr, char* entries) {
+    cudaStream_t stream = c->stream;
     if (n_chunks == 0) return 0;
     const uint32_t ntiles = (uint32_t)ig_gather_tiles(c);
     const int tiles_x = (c->prm.N + IG_GT - 1) / IG_GT;
-    k_gather_plan<<<1, 1024, 0, c->stream>>>(tile_count, tile_off, tile_cur, items, plan_hdr, ntiles);
+    k_gather_plan<<<1, 1024, 0, stream>>>(tile_count, tile_off, tile_cur, items, plan_hdr, ntiles);
     const unsigned sblocks = (unsigned)((n_chunks + 7) / 8);
     switch (c->prm.npol) {
-        case 1: k_gather_scatter<1><<<sblocks, 256, 0, c->stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, entries); break;
-        case 2: k_gather_scatter<2><<<sblocks, 256, 0, c->stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, entries); break;
-        default: k_gather_scatter<4><<<sblocks, 256, 0, c->stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, entries); break;
+        case 1: k_gather_scatter<1><<<sblocks, 256, 0, stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, entries); break;
+        case 2: k_gather_scatter<2><<<sblocks, 256, 0, stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, entries); break;
+        default: k_gather_scatter<4><<<sblocks, 256, 0, stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, entries); break;
     }
-    IG_CUDA_OK(c, cudaMemsetAsync(&c->d_acc->ticket, 0, sizeof(unsigned), c->stream));
+    IG_CUDA_OK(c, cudaMemsetAsync(&c->d_acc->ticket_gather, 0, sizeof(unsigned), stream));
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     dim3 g((unsigned)(sms * IG_GCTAS_PER_SM)), b(IG_GW * 32);
-#define IG_GLAUNCH(P, C) k_gather<P, C><<<g, b, 0, c->stream>>>(entries, items, plan_hdr, c->grid, c->d_bank, c->prm.N, tiles_x, &c->d_acc->ticket, &c->d_acc->commits)
+#define IG_GLAUNCH(P, C) k_gather<P, C><<<g, b, 0, stream>>>(entries, items, plan_hdr, c->grid, c->d_bank, c->prm.N, tiles_x, &c->d_acc->ticket_gather, &c->d_acc->commits)
     if (c->count_commits) {
         switch (c->prm.npol) { case 1: IG_GLAUNCH(1, true); break; case 2: IG_GLAUNCH(2, true); break; default: IG_GLAUNCH(4, true); break; }
     } else {

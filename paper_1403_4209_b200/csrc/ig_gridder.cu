@@ -23,6 +23,9 @@
 // Kernel values come straight from the bank with read-only loads: each (record, tap) value
 // is used once per record, so the only reuse is across records and that lives in L1/L2.
 #include "ig_internal.h"
+#ifndef IG_XP
+#define IG_XP 0          // timing experiments only (results are wrong when non-zero)
+#endif
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -188,7 +191,11 @@ __device__ __forceinline__ unsigned grid_run(const char* __restrict__ rp, int n_
         const bool same = (h.x == last_x) && ((h.z & IG_HDR_WINDOW) == last_z);
         if (same) {
 #pragma unroll
+#if IG_XP == 1
+            for (int k = 0; k < R; ++k) kv[k] = (unsigned long long)(krel[k] + h.y) | (0x3f800000ull << 32);
+#else
             for (int k = 0; k < R; ++k) kv[k] = __ldg(bank64 + (uint32_t)(krel[k] + h.y));
+#endif
         } else {
             last_x = h.x; last_z = h.z & IG_HDR_WINDOW;
             const int cm = IG_HDR_C(h.z), dm = IG_HDR_D(h.z);
@@ -200,19 +207,31 @@ __device__ __forceinline__ unsigned grid_run(const char* __restrict__ rp, int n_
                 const int ty = (int)min((unsigned)tv, (unsigned)(tv - S));
                 pix[k] = (amask & (1u << k)) ? ty * N + ((int)h.x + tx) : -1;
                 krel[k] = (uint32_t)(ty * S + tx);
+#if IG_XP == 1
+                kv[k] = (unsigned long long)(krel[k] + h.y) | (0x3f800000ull << 32);
+#else
                 kv[k] = __ldg(bank64 + (uint32_t)(krel[k] + h.y));            // 32-bit element index
+#endif
             }
 #pragma unroll
             for (int k = 0; k < R; ++k) {
                 // warp-uniform skip: in about half of the (record, slot) pairs no lane's pixel has changed
+#if IG_XP == 3   /* experiment: no commits */
+                prev[k] = pix[k];
+#else
                 if (__any_sync(0xffffffffu, pix[k] != prev[k]))
                     commit_step<NPOL, COUNT>(acc[k], prev[k], pix[k], grid, plane_bytes, n_commit);
+#endif
             }
         }
 #pragma unroll
         for (int k = 0; k < R; ++k) {
+#if IG_XP == 2
+            cmac(acc[k][0], v[0], v[1], kv[k]);
+#else
 #pragma unroll
             for (int q = 0; q < NPOL; ++q) cmac(acc[k][q], v[2 * q], v[2 * q + 1], kv[k]);
+#endif
         }
     }
 #pragma unroll

@@ -42,9 +42,14 @@ __device__ __forceinline__ IgIndex ig_index_one(const IgParams& P, const IgPlane
     if (U > -lim32 && U < lim32 && V > -lim32 && V < lim32) {
         // every record near the grid: the same floor division in 32 bits (a 64-bit divide is ~80 instructions)
         const int nu_ = (int)U + P.shift, nv_ = (int)V + P.shift;
-        int qx = nu_ / P.beta, qy = nv_ / P.beta;
-        if (nu_ - qx * P.beta < 0) qx -= 1;
-        if (nv_ - qy * P.beta < 0) qy -= 1;
+        int qx, qy;
+        if (P.bshift >= 0) {              // beta a power of two: the arithmetic shift is the floor division
+            qx = nu_ >> P.bshift; qy = nv_ >> P.bshift;
+        } else {
+            qx = nu_ / P.beta; qy = nv_ / P.beta;
+            if (nu_ - qx * P.beta < 0) qx -= 1;
+            if (nv_ - qy * P.beta < 0) qy -= 1;
+        }
         x = qx; y = qy;
     } else {
         x = floordiv_ll(U + P.shift, P.beta);
@@ -100,22 +105,32 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
     for (int q = 0; q < NPOL; ++q) nsum[q] = 0.0;
     unsigned long long n_grid = 0, n_drop = 0, n_upd = 0, n_merged = 0;
 
-    // Channels are taken four at a time and their visibilities and weights requested together: a row's four
-    // channels are one 128-byte line (4 pol), so DRAM sees whole lines instead of four separate sector reads.
-    constexpr int CG = 4;
-    for (int c0 = 0; c0 < nchan; c0 += CG) {
-      float4 pre_a[CG], pre_b[CG], pre_w[CG];
-      if constexpr (NPOL == 4) {
+    // Channels are taken two at a time, and the visibilities and weights of the NEXT pair are requested before the
+    // current pair is worked on (two register buffers, loop unrolled by two pairs): a thread's loads are then in
+    // flight all the time instead of only between two ~350-instruction record bodies (ncu: 45 % of the warp time
+    // was spent waiting for them).
+    constexpr int CG = 2;
+    float4 pre_a[2][CG], pre_b[2][CG], pre_w[2][CG];
+    auto prefetch = [&](int buf, int c0) {
+        if constexpr (NPOL == 4) {
 #pragma unroll
-          for (int k = 0; k < CG; ++k) {
-              if (live && c0 + k < nchan) {
-                  const float* vp = vis + ((size_t)row * nchan + c0 + k) * 8;
-                  pre_a[k] = *reinterpret_cast<const float4*>(vp);
-                  pre_b[k] = *reinterpret_cast<const float4*>(vp + 4);
-                  pre_w[k] = *reinterpret_cast<const float4*>(wt + ((size_t)row * nchan + c0 + k) * 4);
-              }
-          }
-      }
+            for (int k = 0; k < CG; ++k) {
+                if (live && c0 + k < nchan) {
+                    const float* vp = vis + ((size_t)row * nchan + c0 + k) * 8;
+                    pre_a[buf][k] = __ldg(reinterpret_cast<const float4*>(vp));
+                    pre_b[buf][k] = __ldg(reinterpret_cast<const float4*>(vp + 4));
+                    pre_w[buf][k] = __ldg(reinterpret_cast<const float4*>(wt + ((size_t)row * nchan + c0 + k) * 4));
+                }
+            }
+        }
+    };
+    prefetch(0, 0);
+    for (int c00 = 0; c00 < nchan; c00 += 2 * CG) {
+#pragma unroll
+     for (int half = 0; half < 2; ++half) {
+      const int c0 = c00 + half * CG;
+      if (c0 >= nchan) break;
+      prefetch(half ^ 1, c0 + CG);
 #pragma unroll
       for (int k = 0; k < CG; ++k) {
         const int c = c0 + k;
@@ -139,9 +154,9 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
             float w[NPOL];
             bool any = false;
             if constexpr (NPOL == 4) {
-                const float4 w4 = pre_w[k];
+                const float4 w4 = pre_w[half][k];
                 w[0] = w4.x; w[1] = w4.y; w[2] = w4.z; w[3] = w4.w;
-                const float4 a = pre_a[k], b = pre_b[k];
+                const float4 a = pre_a[half][k], b = pre_b[half][k];
                 (void)vp; (void)wp;
                 v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
             } else {
@@ -154,8 +169,10 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
                 S = ix.S;
                 const int h = (S - 1) / 2;
                 const int a0 = ix.X - h, b0 = ix.Y - h;
-                int cm = (-a0) % S; if (cm < 0) cm += S;
-                int dm = (-b0) % S; if (dm < 0) dm += S;
+                // (-a0) mod S and (-b0) mod S without integer division: a0, b0 in [0, N), N <= 32768
+                const uint32_t magic = planes[ix.p].magic;
+                const int ra = a0 - (int)__umulhi((uint32_t)a0, magic) * S, rb2 = b0 - (int)__umulhi((uint32_t)b0, magic) * S;
+                const int cm = ra ? S - ra : 0, dm = rb2 ? S - rb2 : 0;
                 const uint32_t tab = (uint32_t)((ix.ov + P.shift) * P.beta + (ix.ou + P.shift));
                 hdr.y = planes[ix.p].koff + tab * (uint32_t)(S * S);
                 is_g = S >= gather_min;
@@ -195,13 +212,15 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
             if (heads != 0xffffffffu) {
                 const uint32_t after = lane == 31 ? 0u : (heads & (0xffffffffu << (lane + 1)));
                 const int end = after ? __ffs(after) - 2 : 31;     // last lane of this lane's group
-#pragma unroll
+                // segmented suffix sum; groups are mostly pairs, so stop as soon as no group is longer than o
+#pragma unroll 1
                 for (int o = 1; o < 32; o <<= 1) {
 #pragma unroll
                     for (int q = 0; q < 2 * NPOL; ++q) {
                         const float t = __shfl_down_sync(0xffffffffu, v[q], o);
                         if (lane + o <= end) v[q] += t;
                     }
+                    if (!__any_sync(0xffffffffu, lane + 2 * o <= end)) break;
                 }
                 if (follows) {
                     hdr.z |= IG_HDR_MERGED;
@@ -242,6 +261,7 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
         unsigned smax = __reduce_max_sync(0xffffffffu, is_g ? 0u : (unsigned)S);
         if (lane == 0 && smax) atomicMax(&chunk_smax[chunk], smax);
       }
+     }
     }
 
     // block reduction of the normaliser and the counters

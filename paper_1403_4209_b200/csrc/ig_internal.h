@@ -30,24 +30,25 @@
 // Large-support record that the fixed-tile gather gridder handles (ig_gather.cu). Its header is
 // {X0 | Y0 << 16, kbase, flags (c = d = S = 0, so the moving-window gridder sees a skip record), S}.
 #define IG_HDR_GATHER (1u << 29)
-#define IG_GATHER_MIN_DEFAULT 17   // supports >= this go to the gather gridder (ig_set_gather_min_support)
+#define IG_GATHER_MIN_DEFAULT 25   // supports >= this go to the gather gridder (ig_set_gather_min_support)
 #define IG_MAX_CHAN_GRIDS 4096   // per-channel grid mode: channels whose normalisers the bank head has room for
 #define IG_GRID_WARPS 4      // warps per gridder CTA
 
 // Device-side tail of the bank buffer: small tables and accumulators.
-struct IgPlaneEntry { int support; uint32_t koff; };   // koff in complex elements
+struct IgPlaneEntry { int support; uint32_t koff; uint32_t magic; uint32_t pad_; };   // koff in complex elements; magic = floor(2^32/S)+1: x/S == umulhi(x, magic) for x < 2^23
 struct IgAccum {
     double norm[4];                     // eq 4.5 normaliser per polarisation
     unsigned long long gridded, dropped, updates;   // eq 4.17
     unsigned long long merged;          // records pre-summed into their predecessor (compression)
     unsigned long long commits;         // pixel commits (atomic reductions of one multi-pol pixel) by the gridder
-    unsigned int ticket;                // work queue of the gridder
-    unsigned int pad_;
+    unsigned int ticket;                // work queue of the moving-window gridder
+    unsigned int ticket_gather;         // work queue of the gather gridder
 };
 
 struct IgParams {            // passed by value to kernels
     int N, beta, P, npol;
     int shift;               // ceil(beta/2) - 1
+    int bshift;              // log2(beta) when beta is a power of two, else -1
     double ku, kw;           // index constants (include/ig.h, DESIGN.md C.1)
 };
 
@@ -79,7 +80,7 @@ struct ig_ctx {
     float2* d_bank = nullptr; double* d_zeta = nullptr; IgPlaneEntry* d_planes = nullptr;
     IgAccum* d_acc = nullptr;
     // timing of the last ig_grid
-    cudaEvent_t ev[IG_TIMING_RING][3] = {};   // ring over the last ig_grid calls
+    cudaEvent_t ev[IG_TIMING_RING][4] = {};   // ring over the last ig_grid calls: start, after ingest, after the moving-window gridder, end
     long long n_timed = 0;                    // ig_grid calls timed so far
     int launches = 0;
     std::string err;
