@@ -25,7 +25,7 @@ bool table_ok(const ig_ctx* c, const int* t) {
         if (t[p] < 1 || t[p] > c->max_support || (t[p] & 1) == 0) return false;
     return true;
 }
-struct GridLayout { size_t freqs, perm, sort, smax, gcount, tile_count, tile_off, tile_cur, plan_hdr, items, records, entries, total; long long nrb, n_chunks; };
+struct GridLayout { size_t freqs, perm, sort, smax, gcount, tile_count, tile_off, tile_cur, plan_hdr, plan_scratch, items, records, entries, total; long long nrb, n_chunks; };
 GridLayout grid_layout(const ig_ctx* c, long long nrow, int nchan) {
     GridLayout L{};
     L.nrb = (nrow + IG_CH - 1) / IG_CH;
@@ -36,11 +36,12 @@ GridLayout grid_layout(const ig_ctx* c, long long nrow, int nchan) {
     L.sort = o; o += ig_align(ig_sort_scratch_bytes(nrow));
     L.smax = o; o += ig_align((size_t)L.n_chunks * 4);
     L.gcount = o; o += ig_align((size_t)L.n_chunks * 4);          // directly after smax (cleared together)
-    const size_t nt = ig_gather_tiles(c);
+    const size_t nt = ig_gather_bins(c);
     L.tile_count = o; o += ig_align(nt * 4);
     L.tile_off = o; o += ig_align(nt * 4);
     L.tile_cur = o; o += ig_align(nt * 4);
     L.plan_hdr = o; o += 256;
+    L.plan_scratch = o; o += ig_align(ig_gather_plan_scratch_bytes(c));
     L.items = o; o += ig_align(ig_gather_max_items(c, L.n_chunks) * 16);
     const size_t rec_bytes = ig_align((size_t)L.n_chunks * IG_CH * ig_rec_stride(c->prm.npol));
     L.records = o; o += rec_bytes;
@@ -269,7 +270,7 @@ ig_status ig_grid(ig_ctx* c, const double* uvw, const int* baseline_id, long lon
     if (any_gather) {
         n = ig_launch_gather(c, records, gcount, L.n_chunks, tile_count, (uint32_t*)(c->work + L.tile_off),
                              (uint32_t*)(c->work + L.tile_cur), (uint4*)(c->work + L.items), (uint32_t*)(c->work + L.plan_hdr),
-                             c->work + L.entries);
+                             c->work + L.entries, (unsigned long long*)(c->work + L.plan_scratch));
         if (n < 0) return IG_ECUDA;
         c->launches += n;
     }

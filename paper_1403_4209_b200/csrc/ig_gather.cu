@@ -30,7 +30,9 @@
 
 #define IG_GT 32          // origin tile side in pixels
 #define IG_GT_SHIFT 5
+#ifndef IG_GCH
 #define IG_GCH 256        // records per gather item
+#endif
 #ifndef IG_GW
 #define IG_GW 8           // warps per gather CTA
 #endif
@@ -53,64 +55,99 @@ __device__ __forceinline__ uint32_t g_lanemask_lt() {
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// plan: tile_count[ntiles] -> tile_off (exclusive scan), tile_cur (= tile_off, the scatter's cursors), items
-// plan_hdr[0] = number of items, [1] = number of entries
-__global__ void __launch_bounds__(1024) k_gather_plan(const uint32_t* __restrict__ tile_count, uint32_t* __restrict__ tile_off,
-                                                      uint32_t* __restrict__ tile_cur, uint4* __restrict__ items,
-                                                      uint32_t* __restrict__ plan_hdr, uint32_t ntiles) {
-    __shared__ unsigned long long wsum[32];
-    __shared__ unsigned long long carry_s;
+// plan: bin_count[nbins] -> bin_off (exclusive scan), bin_cur (= bin_off, the scatter's cursors), items.
+// A bin is (w-plane bucket, origin tile), bucket-major: bin = bucket * ntiles + tile. Items therefore run through the
+// grid one plane bucket at a time, and the CTAs in flight read the kernel matrices of ~P/16 planes only: the part of
+// the bank in use stays in the 126 MB L2 (config 5: 968 MB bank; with tile-only bins the gather kernel missed L2 on
+// a third of its kernel reads and pulled 157 GB from DRAM).
+// Three steps so that many CTAs scan: (a) per block of 4096 bins the totals, (b) one CTA scans the block totals,
+// (c) per block the bins' offsets and items. plan_hdr[0] = number of items, [1] = number of entries.
+__device__ __forceinline__ unsigned long long g_bin_cost(uint32_t c) {       // hi 32 bits: entries, lo 32 bits: items
+    return ((unsigned long long)c << 32) | (unsigned long long)((c + IG_GCH - 1) / IG_GCH);
+}
+// block-wide inclusive scan of one value per thread (1024 threads); returns the inclusive sum, total in *total
+__device__ __forceinline__ unsigned long long g_block_scan(unsigned long long v, unsigned long long* wsum, unsigned long long* total) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) carry_s = 0;
-    __syncthreads();
-    for (uint32_t t0 = 0; t0 < ntiles; t0 += 4096) {
-        const uint32_t i = t0 + threadIdx.x * 4;
-        uint32_t c[4];
-        unsigned long long s = 0;                       // hi 32 bits: entries, lo 32 bits: items
+    unsigned long long inc = v;
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            c[k] = (i + k < ntiles) ? tile_count[i + k] : 0u;
-            s += ((unsigned long long)c[k] << 32) | (unsigned long long)((c[k] + IG_GCH - 1) / IG_GCH);
-        }
-        unsigned long long inc = s;
+    for (int o = 1; o < 32; o <<= 1) {
+        unsigned long long y = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += y;
+    }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        unsigned long long w = wsum[lane], wi = w;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            unsigned long long y = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += y;
+            unsigned long long y = __shfl_up_sync(0xffffffffu, wi, o);
+            if (lane >= o) wi += y;
         }
-        if (lane == 31) wsum[warp] = inc;
-        __syncthreads();
-        if (warp == 0) {
-            unsigned long long w = wsum[lane], wi = w;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                unsigned long long y = __shfl_up_sync(0xffffffffu, wi, o);
-                if (lane >= o) wi += y;
-            }
-            wsum[lane] = wi - w;
-        }
-        __syncthreads();
-        const unsigned long long carry = carry_s;
-        unsigned long long ex = carry + wsum[warp] + (inc - s);
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            if (i + k < ntiles) {
-                const uint32_t off = (uint32_t)(ex >> 32), ioff = (uint32_t)ex;
-                tile_off[i + k] = off;
-                tile_cur[i + k] = off;
-                for (uint32_t j = 0, left = c[k]; left; ++j) {
-                    const uint32_t n = left < IG_GCH ? left : IG_GCH;
-                    items[ioff + j] = make_uint4(i + k, off + j * IG_GCH, n, 0u);
-                    left -= n;
-                }
-            }
-            ex += ((unsigned long long)c[k] << 32) | (unsigned long long)((c[k] + IG_GCH - 1) / IG_GCH);
-        }
-        __syncthreads();
-        if (threadIdx.x == 1023) carry_s = ex;
-        __syncthreads();
+        wsum[lane] = wi - w;               // exclusive over warps
+        if (lane == 31) wsum[32] = wi;     // block total
     }
-    if (threadIdx.x == 0) { plan_hdr[0] = (uint32_t)carry_s; plan_hdr[1] = (uint32_t)(carry_s >> 32); }
+    __syncthreads();
+    const unsigned long long r = inc + wsum[warp];
+    if (total) *total = wsum[32];
+    __syncthreads();
+    return r;
+}
+
+__global__ void __launch_bounds__(1024) k_gather_plan_a(const uint32_t* __restrict__ bin_count, unsigned long long* __restrict__ block_sum,
+                                                        uint32_t nbins) {
+    __shared__ unsigned long long wsum[33];
+    const uint32_t i = blockIdx.x * 4096u + threadIdx.x * 4;
+    unsigned long long s = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) s += g_bin_cost((i + k < nbins) ? bin_count[i + k] : 0u);
+    unsigned long long total;
+    g_block_scan(s, wsum, &total);
+    if (threadIdx.x == 0) block_sum[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(1024) k_gather_plan_b(unsigned long long* __restrict__ block_sum, uint32_t nblocks,
+                                                        uint32_t* __restrict__ plan_hdr) {
+    __shared__ unsigned long long wsum[33];
+    unsigned long long carry = 0;
+    for (uint32_t b0 = 0; b0 < nblocks; b0 += 1024) {
+        const uint32_t i = b0 + threadIdx.x;
+        const unsigned long long v = i < nblocks ? block_sum[i] : 0ull;
+        unsigned long long total;
+        const unsigned long long inc = g_block_scan(v, wsum, &total);
+        if (i < nblocks) block_sum[i] = carry + inc - v;      // exclusive
+        carry += total;
+    }
+    if (threadIdx.x == 0) { plan_hdr[0] = (uint32_t)carry; plan_hdr[1] = (uint32_t)(carry >> 32); }
+}
+
+__global__ void __launch_bounds__(1024) k_gather_plan_c(const uint32_t* __restrict__ bin_count, const unsigned long long* __restrict__ block_sum,
+                                                        uint32_t* __restrict__ bin_off, uint32_t* __restrict__ bin_cur,
+                                                        uint4* __restrict__ items, uint32_t nbins) {
+    __shared__ unsigned long long wsum[33];
+    const uint32_t i = blockIdx.x * 4096u + threadIdx.x * 4;
+    uint32_t c[4];
+    unsigned long long s = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        c[k] = (i + k < nbins) ? bin_count[i + k] : 0u;
+        s += g_bin_cost(c[k]);
+    }
+    const unsigned long long inc = g_block_scan(s, wsum, nullptr);
+    unsigned long long ex = block_sum[blockIdx.x] + inc - s;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        if (i + k < nbins) {
+            const uint32_t off = (uint32_t)(ex >> 32), ioff = (uint32_t)ex;
+            bin_off[i + k] = off;
+            bin_cur[i + k] = off;
+            for (uint32_t j = 0, left = c[k]; left; ++j) {
+                const uint32_t n = left < IG_GCH ? left : IG_GCH;
+                items[ioff + j] = make_uint4(i + k, off + j * IG_GCH, n, 0u);
+                left -= n;
+            }
+        }
+        ex += g_bin_cost(c[k]);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -121,7 +158,7 @@ __global__ void __launch_bounds__(1024) k_gather_plan(const uint32_t* __restrict
 template <int NPOL>
 __global__ void __launch_bounds__(256) k_gather_scatter(const char* __restrict__ records, const uint32_t* __restrict__ gcount,
                                                         long long n_chunks, uint32_t* __restrict__ tile_cur, int tiles_x,
-                                                        char* __restrict__ entries) {
+                                                        uint32_t ntiles, int n_planes, char* __restrict__ entries) {
     constexpr int STRIDE = NPOL == 4 ? 48 : 32;
     constexpr int GSTRIDE = 16 + 16 * NPOL;
     const long long chunk = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
@@ -135,7 +172,8 @@ __global__ void __launch_bounds__(256) k_gather_scatter(const char* __restrict__
         if (!gm) continue;
         if (mine) {
             const int X0 = (int)(h.x & 0xffffu), Y0 = (int)(h.x >> 16);
-            const uint32_t tile = (uint32_t)((Y0 >> IG_GT_SHIFT) * tiles_x + (X0 >> IG_GT_SHIFT));
+            const uint32_t tile = ig_gather_bin((int)(h.z & IG_HDR_GPLANE), n_planes, ntiles,
+                                                (uint32_t)((Y0 >> IG_GT_SHIFT) * tiles_x + (X0 >> IG_GT_SHIFT)));
             const uint32_t peers = __match_any_sync(gm, tile);
             const int leader = __ffs(peers) - 1;
             uint32_t base = 0;
@@ -264,7 +302,7 @@ struct GScan {
 template <int NPOL, bool COUNT>
 __global__ void __launch_bounds__(IG_GW * 32, IG_GCTAS_PER_SM)
 k_gather(const char* __restrict__ entries, const uint4* __restrict__ items, const uint32_t* __restrict__ plan_hdr,
-         float* __restrict__ grid, const float2* __restrict__ bank, int N, int tiles_x, unsigned* __restrict__ ticket,
+         float* __restrict__ grid, const float2* __restrict__ bank, int N, int tiles_x, uint32_t ntiles, unsigned* __restrict__ ticket,
          unsigned long long* __restrict__ commits) {
     constexpr int GSTRIDE = 16 + 16 * NPOL;
     __shared__ __align__(128) char buf[IG_GCH * GSTRIDE];
@@ -309,7 +347,8 @@ k_gather(const char* __restrict__ entries, const uint4* __restrict__ items, cons
         smax = __reduce_max_sync(0xffffffffu, smax);
         const int nsx = (IG_GT - 1 + smax + 7) >> 3, nsy = (IG_GT - 1 + smax + 4 * IG_GR - 1) / (4 * IG_GR);
         const unsigned nsub = (unsigned)(nsx * nsy);
-        const int tile_y = (int)item.x / tiles_x, tile_x = (int)item.x - tile_y * tiles_x;
+        const int tile_id = (int)(item.x % ntiles);        // item.x = plane bucket * ntiles + origin tile
+        const int tile_y = tile_id / tiles_x, tile_x = tile_id - tile_y * tiles_x;
         for (;;) {
             unsigned st = 0;
             if (lane == 0) st = atomicAdd(&s_sub, 1u);
@@ -389,29 +428,35 @@ size_t ig_gather_tiles(const ig_ctx* c) {
     const size_t t = (size_t)((c->prm.N + IG_GT - 1) / IG_GT);
     return t * t;
 }
+size_t ig_gather_bins(const ig_ctx* c) { return ig_gather_tiles(c) * IG_GBUCKETS; }
 size_t ig_gather_max_items(const ig_ctx* c, long long n_chunks) {
-    return (size_t)n_chunks * IG_CH / IG_GCH + ig_gather_tiles(c) + 1;
+    return (size_t)n_chunks * IG_CH / IG_GCH + ig_gather_bins(c) + 1;
 }
+size_t ig_gather_plan_scratch_bytes(const ig_ctx* c) { return ((ig_gather_bins(c) + 4095) / 4096) * 8; }
 
 int ig_launch_gather(ig_ctx* c, const char* records, const uint32_t* gcount, long long n_chunks, uint32_t* tile_count,
-                     uint32_t* tile_off, uint32_t* tile_cur, uint4* items, uint32_t* plan_hdr, char* entries) {
-    cudaStream_t stream = c->stream;
+                     uint32_t* tile_off, uint32_t* tile_cur, uint4* items, uint32_t* plan_hdr, char* entries,
+                     unsigned long long* plan_scratch) {
     if (n_chunks == 0) return 0;
-    const uint32_t ntiles = (uint32_t)ig_gather_tiles(c);
+    cudaStream_t stream = c->stream;
+    const uint32_t ntiles = (uint32_t)ig_gather_tiles(c), nbins = (uint32_t)ig_gather_bins(c);
     const int tiles_x = (c->prm.N + IG_GT - 1) / IG_GT;
-    k_gather_plan<<<1, 1024, 0, stream>>>(tile_count, tile_off, tile_cur, items, plan_hdr, ntiles);
+    const uint32_t nblocks = (nbins + 4095u) / 4096u;
+    k_gather_plan_a<<<nblocks, 1024, 0, stream>>>(tile_count, plan_scratch, nbins);
+    k_gather_plan_b<<<1, 1024, 0, stream>>>(plan_scratch, nblocks, plan_hdr);
+    k_gather_plan_c<<<nblocks, 1024, 0, stream>>>(tile_count, plan_scratch, tile_off, tile_cur, items, nbins);
     const unsigned sblocks = (unsigned)((n_chunks + 7) / 8);
     switch (c->prm.npol) {
-        case 1: k_gather_scatter<1><<<sblocks, 256, 0, stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, entries); break;
-        case 2: k_gather_scatter<2><<<sblocks, 256, 0, stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, entries); break;
-        default: k_gather_scatter<4><<<sblocks, 256, 0, stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, entries); break;
+        case 1: k_gather_scatter<1><<<sblocks, 256, 0, stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, ntiles, c->prm.P, entries); break;
+        case 2: k_gather_scatter<2><<<sblocks, 256, 0, stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, ntiles, c->prm.P, entries); break;
+        default: k_gather_scatter<4><<<sblocks, 256, 0, stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, ntiles, c->prm.P, entries); break;
     }
     IG_CUDA_OK(c, cudaMemsetAsync(&c->d_acc->ticket_gather, 0, sizeof(unsigned), stream));
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     dim3 g((unsigned)(sms * IG_GCTAS_PER_SM)), b(IG_GW * 32);
-#define IG_GLAUNCH(P, C) k_gather<P, C><<<g, b, 0, stream>>>(entries, items, plan_hdr, c->grid, c->d_bank, c->prm.N, tiles_x, &c->d_acc->ticket_gather, &c->d_acc->commits)
+#define IG_GLAUNCH(P, C) k_gather<P, C><<<g, b, 0, stream>>>(entries, items, plan_hdr, c->grid, c->d_bank, c->prm.N, tiles_x, ntiles, &c->d_acc->ticket_gather, &c->d_acc->commits)
     if (c->count_commits) {
         switch (c->prm.npol) { case 1: IG_GLAUNCH(1, true); break; case 2: IG_GLAUNCH(2, true); break; default: IG_GLAUNCH(4, true); break; }
     } else {
@@ -419,5 +464,5 @@ int ig_launch_gather(ig_ctx* c, const char* records, const uint32_t* gcount, lon
     }
 #undef IG_GLAUNCH
     IG_CUDA_OK(c, cudaGetLastError());
-    return 3;
+    return 5;
 }

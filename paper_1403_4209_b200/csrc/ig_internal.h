@@ -30,6 +30,8 @@
 // Large-support record that the fixed-tile gather gridder handles (ig_gather.cu). Its header is
 // {X0 | Y0 << 16, kbase, flags (c = d = S = 0, so the moving-window gridder sees a skip record), S}.
 #define IG_HDR_GATHER (1u << 29)
+#define IG_HDR_GPLANE 0x0003ffffu   // gather records: the w-plane (clamped to 18 bits; only a locality hint for the plan) in the c, d bits of word z, S stays 0
+#define IG_GBUCKETS 16             // w-plane buckets of the gather plan: bin = bucket * tiles + origin tile
 #define IG_GATHER_MIN_DEFAULT 25   // supports >= this go to the gather gridder (ig_set_gather_min_support)
 #define IG_MAX_CHAN_GRIDS 4096   // per-channel grid mode: channels whose normalisers the bank head has room for
 #define IG_GRID_WARPS 4      // warps per gridder CTA
@@ -102,9 +104,16 @@ int ig_launch_index(ig_ctx* c, const double* uvw, const uint32_t* perm, long lon
                     char* records, uint32_t* chunk_smax, uint32_t* gcount, uint32_t* tile_count, int gather_min);   // uses c->per_channel / c->d_chan_norm
 // gather gridder (ig_gather.cu): plan, scatter, gridder; gcount[chunk] = marked records per work item
 size_t ig_gather_tiles(const ig_ctx* c);
+size_t ig_gather_bins(const ig_ctx* c);
+size_t ig_gather_plan_scratch_bytes(const ig_ctx* c);
+// plan bin of a gather record (both k_index and k_gather_scatter call it)
+__host__ __device__ static inline uint32_t ig_gather_bin(int plane, int n_planes, uint32_t ntiles, uint32_t tile) {
+    return (uint32_t)(((long long)plane * IG_GBUCKETS) / n_planes) * ntiles + tile;
+}
 size_t ig_gather_max_items(const ig_ctx* c, long long n_chunks);
 int ig_launch_gather(ig_ctx* c, const char* records, const uint32_t* gcount, long long n_chunks, uint32_t* tile_count,
-                     uint32_t* tile_off, uint32_t* tile_cur, uint4* items, uint32_t* plan_hdr, char* entries);
+                     uint32_t* tile_off, uint32_t* tile_cur, uint4* items, uint32_t* plan_hdr, char* entries,
+                     unsigned long long* plan_scratch);
 int ig_launch_debug_index(ig_ctx* c, const double* uvw, long long nrow, const double* d_freqs, int nchan,
                           int* X, int* Y, int* ou, int* ov, int* pl, int* fl);
 int ig_launch_gridder(ig_ctx* c, const char* records, const uint32_t* chunk_smax, long long nrb, int nchan);
