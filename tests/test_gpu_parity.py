@@ -44,6 +44,9 @@ CASES = {
     "pol2": small(synth.CONFIGS[1], n_pol=2, n_station=9, n_time=77, n_chan=3, n_wplanes=8),
     # grid side that is not a power of two (the thesis images 4500^2, :1988), odd row count, 1 polarisation
     "n300": small(synth.CONFIGS[1], grid_n=300, n_pol=1, n_station=7, n_time=61, n_chan=2, n_wplanes=5, s_max=21),
+    # oversampling that is not a power of two (the index kernel's division path), 2 polarisations, supports on both sides
+    # of the gather threshold
+    "beta3": small(synth.CONFIGS[1], oversampling=3, n_pol=2, n_station=8, n_time=60, n_chan=3, n_wplanes=6, s_max=31),
 }
 
 
