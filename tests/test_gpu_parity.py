@@ -698,3 +698,27 @@ def test_stokes_output_matches_oracle(npol, orc, torch_cuda):
     assert np.abs(got[:, b0 + n // 2, a0 + n // 2] - [I, Q, U, V][:npol]).max() < 2e-2
     if npol > 1:        # the switch changed the output: the plain images are the correlations
         assert np.abs(plain.cpu().numpy()[0, b0 + n // 2, a0 + n // 2] - (I + Q)) < 2e-2
+
+
+@pytest.mark.parametrize("name,threshold", [("cfg2s", 1), ("cfg5s", 1), ("cfg5s", 1000), ("cfg4s", 13), ("pol2", 1), ("n300", 1)])
+def test_both_work_distributions_give_the_oracle_grid(name, threshold, runs, torch_cuda):
+    """ig_set_gather_min_support moves records between the moving-window gridder and the fixed-tile gather gridder
+    (include/ig.h): everything through the gather kernel (threshold 1, supports down to 7), everything through the
+    moving window (threshold above IG_MAX_SUPPORT, supports up to 129), and a threshold inside the support range all
+    reproduce the oracle's grid, statistics and normaliser; the gridder-time split adds up."""
+    wl, ref = runs(name)
+    g = make_gridder(wl)
+    g.debug_set_wkernels(wl["w_max"], ref["bank"].astype(np.complex64))
+    g.set_gather_min_support(threshold)
+    g.set_commit_counting(True)
+    uvw, bl, vis, wt = to_dev(torch_cuda, wl)
+    g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+    check_grid(g.grid_complex(), ref["grid"])
+    assert g.stats() == tuple(int(x) for x in ref["stats"])
+    _, norm = g.finalize()
+    assert np.allclose(norm, ref["norm"], rtol=1e-6, atol=0)
+    ingest_ms, gridder_ms = g.timing()
+    window_ms, gather_ms = g.gridder_split()
+    assert ingest_ms > 0 and gridder_ms > 0 and window_ms >= 0 and gather_ms >= 0
+    assert abs((window_ms + gather_ms) - gridder_ms) <= 0.05 * gridder_ms + 0.02
+    assert g.commits() > 0
