@@ -145,10 +145,8 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
         bool is_g = false;                // large support: goes to the gather gridder (ig_gather.cu)
         uint32_t g_tile = 0;
         double cn[NPOL];                  // this record's normaliser terms (per-channel grid mode)
-        double zsum = 0.0;                // sum of the record's kernel matrix (eq 4.3)
-        float wn[NPOL];                   // weights of a gridded record, 0 otherwise
 #pragma unroll
-        for (int q = 0; q < NPOL; ++q) wn[q] = 0.f;
+        for (int q = 0; q < NPOL; ++q) cn[q] = 0.0;
         if (live) {
             IgIndex ix = ig_index_one(P, planes, um, vm, wm, freqs[c]);
             const float* vp = vis + ((size_t)row * nchan + c) * (2 * NPOL);
@@ -190,11 +188,11 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
                     hdr.z = IG_HDR_PACK(cm, dm, S) | (conj ? IG_HDR_CONJ : 0u);
                     hdr.w = (uint32_t)ix.p;
                 }
-                // the kernel-sum load is requested here and used after the record is written (it comes from L2)
-                zsum = __ldg(&zeta[(size_t)ix.p * P.beta * P.beta + tab]);
+                const double z = zeta[(size_t)ix.p * P.beta * P.beta + tab];
 #pragma unroll
                 for (int q = 0; q < NPOL; ++q) {
-                    wn[q] = w[q];
+                    cn[q] = (double)w[q] * z;
+                    nsum[q] += cn[q];                         // eq 4.5
                     v[2 * q] = w[q] * v[2 * q];               // eq 4.16
                     v[2 * q + 1] = conj ? -(w[q] * v[2 * q + 1]) : w[q] * v[2 * q + 1];
                 }
@@ -242,11 +240,6 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
             *reinterpret_cast<float4*>(rec + 16) = make_float4(v[0], v[1], v[2], v[3]);
         } else {
             *reinterpret_cast<float4*>(rec + 16) = make_float4(v[0], v[1], 0.f, 0.f);
-        }
-#pragma unroll
-        for (int q = 0; q < NPOL; ++q) {
-            cn[q] = (double)wn[q] * zsum;
-            nsum[q] += cn[q];                                 // eq 4.5
         }
         if (chan_norm) {                  // one grid per channel: eq 4.5 per channel
 #pragma unroll
