@@ -15,6 +15,12 @@
 // item, dropped records stay as 16-byte "skip" headers (S = 0), and the only plan datum
 // is the largest support per item. No scan, no host round trip.
 #include "ig_internal.h"
+#ifndef IG_INDEX_CG
+#define IG_INDEX_CG 2        // channels whose visibilities are requested together (two such groups are in flight)
+#endif
+#ifndef IG_INDEX_CTAS
+#define IG_INDEX_CTAS 4      // resident CTAs per SM the register allocation aims at
+#endif
 
 struct IgIndex { int X, Y, ou, ov, p, S, on; };
 
@@ -79,7 +85,7 @@ __device__ __forceinline__ IgIndex ig_index_one(const IgParams& P, const IgPlane
 // Record at place ((rb*nchan + c)*IG_CH + t): 16-byte header {pix_base, kbase, z = c | d<<9 | S<<18 | flags (ig_internal.h), plane}
 // followed by npol complex32 pairs (stride 48 B for 4 pol, else 32 B).
 template <int NPOL>
-__global__ void __launch_bounds__(IG_CH)
+__global__ void __launch_bounds__(IG_CH, IG_INDEX_CTAS)
 k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __restrict__ zeta,
         const double* __restrict__ uvw, const uint32_t* __restrict__ perm, long long nrow,
         const double* __restrict__ freqs, int nchan, const float* __restrict__ vis,
@@ -109,7 +115,7 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
     // current pair is worked on (two register buffers, loop unrolled by two pairs): a thread's loads are then in
     // flight all the time instead of only between two ~350-instruction record bodies (ncu: 45 % of the warp time
     // was spent waiting for them).
-    constexpr int CG = 2;
+    constexpr int CG = IG_INDEX_CG;
     float4 pre_a[2][CG], pre_b[2][CG], pre_w[2][CG];
     auto prefetch = [&](int buf, int c0) {
         if constexpr (NPOL == 4) {
