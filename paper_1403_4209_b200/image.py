@@ -3,7 +3,7 @@ from an .npz file (keys uvw_m [nrow,3] f64 metres, baseline [nrow] i32, freqs_hz
 weights [nrow,nchan,npol] f32). Writes the dirty image(s) [npol][N][N] float32 as .npy (the thesis writes FITS, :1680-1687;
 no FITS library is assumed here).
 
-    python -m paper_1403_4209_b200.image --config 2 --out dirty.npy
+    python -m paper_1403_4209_b200.image --config 2 --stokes --out dirty.npy
     python -m paper_1403_4209_b200.image --npz data.npz --grid 2048 --cell-arcsec 14.57 --wplanes 64 --max-support 65 --out dirty.npy
 """
 from __future__ import annotations
@@ -26,6 +26,7 @@ def main():
     ap.add_argument("--wplanes", type=int, default=1)
     ap.add_argument("--oversampling", type=int, default=8)
     ap.add_argument("--max-support", type=int, default=33)
+    ap.add_argument("--stokes", action="store_true", help="write Stokes I,Q,U,V images (Alg 4.6 step 2) instead of the polarisations")
     ap.add_argument("--out", default="dirty.npy")
     a = ap.parse_args()
     build.build()
@@ -49,6 +50,7 @@ def main():
     g.allocate(sup)
     g.build_wkernels(w_max if P > 1 else 0.0)
     g.grid_visibilities_host(wl["uvw_m"], wl["baseline"], wl["freqs_hz"], np.ascontiguousarray(wl["vis"]), wl["weights"])
+    g.set_stokes_output(a.stokes)
     img, norm = g.finalize()
     gridded, dropped, updates = g.stats()
     np.save(a.out, img.cpu().numpy())

@@ -722,3 +722,46 @@ def test_both_work_distributions_give_the_oracle_grid(name, threshold, runs, tor
     assert ingest_ms > 0 and gridder_ms > 0 and window_ms >= 0 and gather_ms >= 0
     assert abs((window_ms + gather_ms) - gridder_ms) <= 0.05 * gridder_ms + 0.02
     assert g.commits() > 0
+
+
+def test_command_line_tools_run(tmp_path, orc, torch_cuda):
+    """The two user-facing scripts over the C ABI: the headless imager on arrays from an .npz file (automatic supports,
+    Stokes output) reproduces the oracle's Stokes image of the same data, and the fixed-support sweep prints one JSON line
+    per point with consistent counts."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    cfg = small(synth.CONFIGS[1], grid_n=256, n_station=8, n_time=40, n_chan=2, n_wplanes=6)
+    wl = synth.make_workload(cfg)
+    npz = tmp_path / "vis.npz"
+    np.savez(npz, uvw_m=wl["uvw_m"], baseline=wl["baseline"], freqs_hz=wl["freqs_hz"], vis=wl["vis"], weights=wl["weights"])
+    out = tmp_path / "dirty.npy"
+    cell_arcsec = np.degrees(wl["cell_rad"]) * 3600.0
+    r = subprocess.run([sys.executable, "-m", "paper_1403_4209_b200.image", "--npz", str(npz), "--grid", str(cfg.grid_n),
+                        "--cell-arcsec", repr(float(cell_arcsec)), "--wplanes", str(cfg.n_wplanes), "--max-support", "31",
+                        "--stokes", "--out", str(out)], cwd=root, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    img = np.load(out)
+    assert img.shape == (cfg.n_pol, cfg.grid_n, cfg.grid_n) and np.isfinite(img).all()
+    # the same through the oracle: automatic supports, bank, grid, Stokes finaliser
+    cell = np.radians(cell_arcsec / 3600.0)
+    du = 1.0 / (cfg.grid_n * cell)
+    w_max = float(np.abs(wl["uvw_m"][:, 2]).max() * wl["freqs_hz"].max() / synth.C_M_S)
+    sup = orc.auto_supports(cfg.n_wplanes, w_max, du, cfg.oversampling, 31)
+    bank, off = orc.build_bank(sup, w_max, du, cfg.oversampling, 31)
+    idx = orc.index_records(wl["uvw_m"], wl["freqs_hz"], cfg.grid_n, cell, cfg.oversampling, cfg.n_wplanes, w_max, sup)
+    gr, nrm, _ = orc.grid_records(idx, wl["vis"], wl["weights"], cfg.grid_n, cfg.oversampling, sup, bank, off)
+    want = orc.finalize_stokes(gr, nrm, cfg.oversampling)
+    n = cfg.grid_n
+    inner = slice(n // 8, n - n // 8)
+    assert np.abs(img[:, inner, inner] - want[:, inner, inner]).max() <= 2e-4 * np.abs(want[:, inner, inner]).max()
+
+    r = subprocess.run([sys.executable, "-m", "paper_1403_4209_b200.sweep", "--config", "1", "--supports", "7,31", "--betas", "2",
+                        "--pols", "1,2", "--steps", "1"], cwd=root, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [json.loads(x) for x in r.stdout.splitlines() if x.startswith("{")]
+    assert [(d["support"], d["n_pol"]) for d in lines] == [(7, 1), (31, 1), (7, 2), (31, 2)]
+    for d in lines:
+        assert d["records_gridded"] + d["records_dropped"] == 1792 and d["updates_per_s"] > 0
+        assert (d["gather_ms"] > d["window_ms"]) == (d["support"] >= 25)
