@@ -44,6 +44,7 @@ def parse():
     ap.add_argument("--no-compress", action="store_true", help="switch compression off (thesis: real vs total rate)")
     ap.add_argument("--host-slices", type=int, default=8, help="ig_grid_host: slices copied while the previous one is gridded")
     ap.add_argument("--gather-min-support", type=int, default=None, help="ig_set_gather_min_support (experiments)")
+    ap.add_argument("--sort-tile-shift", type=int, default=None, help="ig_set_sort_tile_shift (experiments)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="time only --config (default: configs 1-4 too, after the main one)")
@@ -286,6 +287,8 @@ def bench_config(args, config, dev, ranks, steps, warmup, want_e2e, fp32_peak, c
     g.set_compression(not args.no_compress)
     if args.gather_min_support is not None:
         g.set_gather_min_support(args.gather_min_support)
+    if args.sort_tile_shift is not None:
+        g.set_sort_tile_shift(args.sort_tile_shift)
 
     vis_f = np.ascontiguousarray(wl["vis"]).view(np.float32).reshape(nrow, nchan, npol, 2)
     host = dict(uvw=wl["uvw_m"], bl=wl["baseline"], vis=vis_f, wt=wl["weights"])
