@@ -244,7 +244,7 @@ template <int NPOL, bool COUNT>
 __global__ void __launch_bounds__(IG_GRID_WARPS * 32, IG_GRID_CTAS_PER_SM)
 k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_smax, unsigned nrb, unsigned nchan,
           float* __restrict__ grid, const float2* __restrict__ bank, int N, unsigned* __restrict__ ticket,
-          unsigned long long* __restrict__ commits, size_t chan_stride) {
+          unsigned long long* __restrict__ commits, size_t chan_stride, bool two_phase) {
     constexpr int STRIDE = NPOL == 4 ? 48 : 32;
     constexpr int STAGE_BYTES = IG_STAGE * STRIDE;
     __shared__ __align__(128) char sm_rec[IG_GRID_WARPS][IG_CH * STRIDE];
@@ -267,12 +267,18 @@ k_gridder(const char* __restrict__ records, const uint32_t* __restrict__ chunk_s
         unsigned tk = 0;
         if (lane == 0) tk = atomicAdd(ticket, 1u);
         tk = __shfl_sync(0xffffffffu, tk, 0);
-        if (tk >= n_chunks) break;
+        // Small batches (two_phase): the queue is walked twice, first the items with multi-pass supports, then the rest, so
+        // that the expensive items are not left for the end (longest-first; matters when a warp gets only tens of items)
+        if (tk >= (two_phase ? 2u * n_chunks : n_chunks)) break;
+        const bool second = tk >= n_chunks;
+        const unsigned ti = second ? tk - n_chunks : tk;
         // tickets run channel-major: neighbours in the queue are neighbouring row blocks of ONE channel
-        const unsigned ch = tk / nrb;
-        const unsigned chunk = (tk - ch * nrb) * nchan + ch;
+        const unsigned ch = ti / nrb;
+        const unsigned chunk = (ti - ch * nrb) * nchan + ch;
         float* __restrict__ grid_ch = grid + (size_t)ch * chan_stride;   // per-channel grids: chan_stride = floats per grid, else 0
-        if (chunk_smax[chunk] == 0) continue;          // every record of the item was dropped
+        const unsigned sm_item = chunk_smax[chunk];
+        if (sm_item == 0) continue;                    // every record of the item was dropped
+        if (two_phase && ((sm_item >= 13u) == second)) continue;
         __syncwarp();                                  // all lanes are done with the previous item
         if (lane == 0) {
             const char* src = records + (size_t)chunk * (IG_CH * STRIDE);
@@ -361,7 +367,8 @@ int ig_launch_gridder(ig_ctx* c, const char* records, const uint32_t* chunk_smax
     long long want = (n_chunks + IG_GRID_WARPS - 1) / IG_GRID_WARPS;
     unsigned ctas = (unsigned)(want < (long long)sms * per_sm ? want : (long long)sms * per_sm);
     dim3 g(ctas), b(IG_GRID_WARPS * 32);
-#define IG_LAUNCH(P, C) k_gridder<P, C><<<g, b, 0, c->stream>>>(records, chunk_smax, (unsigned)nrb, (unsigned)nchan, c->grid, c->d_bank, c->prm.N, &c->d_acc->ticket, &c->d_acc->commits, c->per_channel ? (size_t)c->prm.N * c->prm.N * c->prm.npol * 2 : (size_t)0)
+    const bool two_phase = n_chunks < 200ll * ctas * IG_GRID_WARPS && n_chunks < (1ll << 30);   // fewer than ~200 items per warp
+#define IG_LAUNCH(P, C) k_gridder<P, C><<<g, b, 0, c->stream>>>(records, chunk_smax, (unsigned)nrb, (unsigned)nchan, c->grid, c->d_bank, c->prm.N, &c->d_acc->ticket, &c->d_acc->commits, c->per_channel ? (size_t)c->prm.N * c->prm.N * c->prm.npol * 2 : (size_t)0, two_phase)
     if (c->count_commits) {
         switch (c->prm.npol) { case 1: IG_LAUNCH(1, true); break; case 2: IG_LAUNCH(2, true); break; default: IG_LAUNCH(4, true); break; }
     } else {
