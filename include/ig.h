@@ -132,6 +132,30 @@ ig_status ig_set_host_slices(ig_ctx* ctx, int n);
 ig_status ig_grid_host(ig_ctx* ctx, const double* uvw_m, const int* baseline_id, long long nrow,
                        const double* freqs_hz, int nchan, const float* vis, const float* weights);
 
+/* ig_grid for a caller that cannot allocate device memory. ig_grid needs a work_dev sized per batch, which
+ * somebody must cudaMalloc. A gridding stage that runs inside someone else's process (a correlator pipeline, a
+ * framework that has reserved all of HBM for its own pool and hands out fixed input and output buffers), or
+ * inside a latency-bound loop where cudaMalloc / cudaFree would stall the whole device, has nobody to ask.
+ * This call is ig_grid with its scratch in an array that is part of the library itself (a file-scope
+ * __device__ array in csrc/ig_static.cu): same arguments (eq 4.4, steps A1-A3 and C as above), same result up to
+ * fp32 summation order, and neither it nor anything it calls allocates or frees device or host memory.
+ *   - Limit: ig_workspace_bytes(ctx, nrow, nchan) <= IG_STATIC_WORK_BYTES (32 MiB; e.g. ~230 000 four-polarisation
+ *     records on a 2048^2 grid). A larger batch returns IG_ENOMEM, text in ig_last_error, nothing enqueued: feed
+ *     smaller batches (ig_grid* calls add up) or use ig_grid.
+ *   - Cost: each GPU this call runs on holds those 32 MiB from the first call until the process exits.
+ *   - First call on a GPU: looks up where the array sits on that GPU (once per device, cached; the context's device
+ *     must be current, IG_EINVAL if the bound grid lives elsewhere). Make that first call during set-up, before
+ *     any stream capture is begun.
+ *   - The array is shared by EVERY call on that GPU, whatever the context, and keeps the last call's bytes. The call
+ *     clears what it counts in, so calls on one stream may follow each other freely; two calls that can run at the
+ *     same time on the GPU (different streams, different host threads' contexts) overwrite each other's
+ *     scratch and give wrong grids - order them with events, or give all but one a work buffer and ig_grid.
+ *   - ig_bind still asks for a work_dev (the bank builder and the finaliser use it); this call never touches it.
+ * The bound work buffer, the statistics, the timing ring and ig_last_launches behave as after ig_grid. */
+#define IG_STATIC_WORK_BYTES (32u << 20)
+ig_status ig_grid_static(ig_ctx* ctx, const double* uvw_m, const int* baseline_id, long long nrow,
+                         const double* freqs_hz, int nchan, const float* vis, const float* weights);
+
 /* Algorithm 4.6: inverse FFT per polarisation (uv origin at pixel (N/2,N/2), +j sign,
  * unnormalised, eq 2.8 :516), real part divided by the normaliser (eq 4.5), the taper
  * (eq 2.9) and the sinc of the nearest-sample lookup (eq 2.13). By default the images are the polarisations

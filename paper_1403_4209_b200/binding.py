@@ -14,6 +14,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
+IG_STATIC_WORK_BYTES = 32 << 20    # include/ig.h: scratch built into the library for ig_grid_static
 STATUS = {0: "IG_OK", 1: "IG_EINVAL", 2: "IG_ESTATE", 3: "IG_ECUDA", 4: "IG_ENOMEM", 5: "IG_EUNSUPPORTED"}
 
 _vp, _sz, _ll, _i, _d = C.c_void_p, C.c_size_t, C.c_longlong, C.c_int, C.c_double
@@ -32,6 +33,7 @@ SIGNATURES = {
     "ig_debug_set_wkernels": (_i, [_vp, _d, _vp, _vp, _sz]),
     "ig_debug_get_wkernels": (_i, [_vp, _vp, _sz]),
     "ig_grid": (_i, [_vp, _vp, _vp, _ll, _vp, _i, _vp, _vp]),
+    "ig_grid_static": (_i, [_vp, _vp, _vp, _ll, _vp, _i, _vp, _vp]),
     "ig_host_staging_bytes": (_sz, [_vp, _ll, _i]),
     "ig_set_host_slices": (_i, [_vp, _i]),
     "ig_grid_host": (_i, [_vp, _vp, _vp, _ll, _vp, _i, _vp, _vp]),
@@ -231,6 +233,16 @@ class Gridder:
         self.ensure_work(self.workspace_bytes(nrow, nchan))
         self._check(self.lib.ig_grid(self.ctx, _vp(uvw_m.data_ptr()), _vp(baseline_id.data_ptr()), nrow,
                                      _np_ptr(freqs), nchan, _vp(vis.data_ptr()), _vp(weights.data_ptr())), "ig_grid")
+
+    def grid_visibilities_static(self, uvw_m, baseline_id, freqs_hz, vis, weights):
+        """ig_grid_static: same arguments and result as grid_visibilities, but the scratch is the library's built-in
+        32 MiB device array instead of a work buffer, so nothing is allocated here or in the library. For callers
+        that may not touch the device heap (see include/ig.h). Raises IgError (IG_ENOMEM) when the batch is too large."""
+        freqs = np.ascontiguousarray(freqs_hz, dtype=np.float64)
+        nrow, nchan = int(uvw_m.shape[0]), int(freqs.size)
+        self._check_inputs(uvw_m, baseline_id, vis, weights, nrow, nchan, on_device=True)
+        self._check(self.lib.ig_grid_static(self.ctx, _vp(uvw_m.data_ptr()), _vp(baseline_id.data_ptr()), nrow,
+                                            _np_ptr(freqs), nchan, _vp(vis.data_ptr()), _vp(weights.data_ptr())), "ig_grid_static")
 
     def grid_visibilities_host(self, uvw_m, baseline_id, freqs_hz, vis, weights):
         """Same with HOST buffers (numpy arrays or pinned CPU torch tensors): the end-to-end call."""

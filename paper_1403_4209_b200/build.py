@@ -6,7 +6,7 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["ig_api.cu", "ig_sort.cu", "ig_ingest.cu", "ig_gridder.cu", "ig_gather.cu", "ig_bank.cu", "ig_finalize.cu", "ig_micro.cu"]
+SOURCES = ["ig_api.cu", "ig_sort.cu", "ig_ingest.cu", "ig_gridder.cu", "ig_gather.cu", "ig_bank.cu", "ig_finalize.cu", "ig_micro.cu", "ig_static.cu"]
 LIB = os.path.join(HERE, "libig.so")
 CUDA_HOME = os.environ.get("CUDA_HOME", "/usr/local/cuda")
 

@@ -61,6 +61,11 @@ def test_create_validates_arguments(lib):
     assert lib.ig_build_wkernels(ctx, 10.0, sup.ctypes.data_as(ctypes.c_void_p)) == 2
     assert lib.ig_grid(ctx, None, None, 0, None, 1, None, None) == 2
     assert b"ig_bind" in lib.ig_last_error(ctx)
+    # the no-allocation entry point follows the same state machine, and the binding's copy of its limit is the header's
+    assert lib.ig_grid_static(ctx, None, None, 0, None, 1, None, None) == 2
+    from paper_1403_4209_b200 import binding
+    m = re.search(r"#define\s+IG_STATIC_WORK_BYTES\s+\((\d+)u\s*<<\s*(\d+)\)", open(os.path.join(ROOT, "include", "ig.h")).read())
+    assert m and int(m.group(1)) << int(m.group(2)) == binding.IG_STATIC_WORK_BYTES
     lib.ig_destroy(ctx)
 
 
