@@ -64,7 +64,14 @@ int install_table(ig_ctx* c, const int* table) {
     c->bank_elems = e;
     if (bank_head_bytes(c) + e * 8 > c->bank_bytes) { c->err = "bank buffer too small (see ig_bank_bytes)"; return -2; }
     std::vector<IgPlaneEntry> pe(P);
-    for (int p = 0; p < P; ++p) { pe[p].support = table[p]; pe[p].koff = c->koff[p]; pe[p].magic = (uint32_t)((1ull << 32) / (unsigned)table[p]) + 1u; pe[p].pad_ = 0u; }
+    for (int p = 0; p < P; ++p) {
+        pe[p].support = table[p];
+        pe[p].koff = c->koff[p];
+        // floor(2^32/S)+1 does not fit 32 bits for S = 1; 2^32-1 there gives x - umulhi(x, magic) = 1 for x > 0 (0 for
+        // x = 0), which k_index turns into c = S - 1 = 0: the right answer, since x mod 1 = 0
+        pe[p].magic = table[p] == 1 ? 0xffffffffu : (uint32_t)((1ull << 32) / (unsigned)table[p]) + 1u;
+        pe[p].pad_ = 0u;
+    }
     IG_CUDA_OK(c, cudaMemcpyAsync(c->d_planes, pe.data(), (size_t)P * sizeof(IgPlaneEntry), cudaMemcpyHostToDevice, c->stream));
     IG_CUDA_OK(c, cudaStreamSynchronize(c->stream));
     return 0;

@@ -37,7 +37,7 @@
 #define IG_GRID_WARPS 4      // warps per gridder CTA
 
 // Device-side tail of the bank buffer: small tables and accumulators.
-struct IgPlaneEntry { int support; uint32_t koff; uint32_t magic; uint32_t pad_; };   // koff in complex elements; magic = floor(2^32/S)+1: x/S == umulhi(x, magic) for x < 2^23
+struct IgPlaneEntry { int support; uint32_t koff; uint32_t magic; uint32_t pad_; };   // koff in complex elements; magic = floor(2^32/S)+1: x/S == umulhi(x, magic) for x < 2^23 (S = 1: 2^32-1, see install_table)
 struct IgAccum {
     double norm[4];                     // eq 4.5 normaliser per polarisation
     unsigned long long gridded, dropped, updates;   // eq 4.17

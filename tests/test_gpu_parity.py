@@ -64,6 +64,14 @@ def make_gridder(wl):
     return g
 
 
+def make_gridder_max(wl, max_support):
+    from paper_1403_4209_b200.binding import Gridder
+    cfg = wl["cfg"]
+    g = Gridder(cfg.grid_n, wl["cell_rad"], cfg.n_wplanes, cfg.oversampling, max_support, cfg.n_pol)
+    g.allocate(wl["supports"])
+    return g
+
+
 def oracle_run(orc, wl, bank=None, bank_off=None):
     cfg = wl["cfg"]
     sup = wl["supports"]
@@ -722,6 +730,41 @@ def test_both_work_distributions_give_the_oracle_grid(name, threshold, runs, tor
     assert ingest_ms > 0 and gridder_ms > 0 and window_ms >= 0 and gather_ms >= 0
     assert abs((window_ms + gather_ms) - gridder_ms) <= 0.05 * gridder_ms + 0.02
     assert g.commits() > 0
+
+
+@pytest.mark.parametrize("threshold", [1000, 1, 5])
+@pytest.mark.parametrize("npol", [1, 2, 4])
+def test_smallest_supports(npol, threshold, orc, torch_cuda):
+    """Supports 1, 3 and 5 (include/ig.h: odd, 1..max_support), alone in a plane and mixed with 7 and 9
+    inside one work item, through the moving window (one point per lane, R = 1), the gather gridder, and a threshold
+    that splits them. S = 1 is the edge of the magic-number modulo of the record header (c = d = 0 for every cell)."""
+    cfg = small(synth.CONFIGS[1], grid_n=512, n_pol=npol, n_station=9, n_time=90, n_chan=3, n_wplanes=8, s_min=1, s_max=9)
+    wl = synth.make_workload(cfg)
+    wl["supports"] = np.array([1, 3, 5, 7, 9, 3, 1, 5], dtype=np.int32)
+    ref = oracle_run(orc, wl)
+    planes, counts = np.unique(ref["idx"]["plane"][(ref["idx"]["flags"] & 2) != 0], return_counts=True)
+    assert set(planes) >= {0, 1, 2, 5, 6, 7} and counts.min() >= 20      # every small support is really gridded
+    g = make_gridder(wl)
+    g.debug_set_wkernels(wl["w_max"], ref["bank"].astype(np.complex64))
+    g.set_gather_min_support(threshold)
+    uvw, bl, vis, wt = to_dev(torch_cuda, wl)
+    g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+    check_grid(g.grid_complex(), ref["grid"])
+    assert g.stats() == tuple(int(x) for x in ref["stats"])
+    _, norm = g.finalize()
+    assert np.allclose(norm, ref["norm"], rtol=1e-6, atol=0)
+    # a table of nothing but 1: plain nearest-cell gridding
+    wl["supports"] = np.ones(8, dtype=np.int32)
+    rng = np.random.default_rng(11)
+    b2 = cfg.oversampling ** 2
+    bank = (rng.standard_normal(8 * b2) + 1j * rng.standard_normal(8 * b2)).astype(np.complex64).astype(np.complex128)
+    ref = oracle_run(orc, wl, bank=bank, bank_off=np.arange(8, dtype=np.int64) * b2)
+    g = make_gridder_max(wl, 3)
+    g.debug_set_wkernels(wl["w_max"], ref["bank"].astype(np.complex64))
+    g.set_gather_min_support(threshold)
+    g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+    check_grid(g.grid_complex(), ref["grid"])
+    assert g.stats() == tuple(int(x) for x in ref["stats"])
 
 
 def test_command_line_tools_run(tmp_path, orc, torch_cuda):
