@@ -283,13 +283,18 @@ def finalize(grid, norm, beta):
 #   4 pol: I = (D_XX + D_YY)/2, Q = (D_XX - D_YY)/2, U = (D_XY + D_YX)/2, V = (D_XY - D_YX)/(2j)
 #   2 pol (XX, YY): I, Q as above;   1 pol: I = D_0 (the only Stokes "that can be calculated", :1660).
 # The real part is taken after the combination (V needs the imaginary parts), then steps 3-4 as finalize.
+# A polarisation whose normaliser is zero was flagged throughout (eq 4.5 sums weights x kernel sums, :1286), its
+# grid is identically zero, and 0/0 has no value: it enters the combinations as D_p = 0 (reading 21).
 def finalize_stokes(grid, norm, beta):
     n, npol = grid.shape[0], grid.shape[2]
     a = np.arange(-n // 2, n // 2, dtype=np.float64)
     psi = taper(2.0 * a / n)
     snc = np.sinc(a / (n * beta))
     corr = np.outer(psi * snc, psi * snc)
-    d = transform_grid(grid) / np.asarray(norm, dtype=np.float64)[:, None, None]
+    nrm = np.asarray(norm, dtype=np.float64)
+    d = transform_grid(grid)
+    for p in range(npol):
+        d[p] = d[p] / nrm[p] if nrm[p] != 0.0 else 0.0
     if npol == 4:
         st = np.stack([(d[0] + d[3]) / 2, (d[0] - d[3]) / 2, (d[1] + d[2]) / 2, (d[1] - d[2]) / 2j])
     elif npol == 2:

@@ -102,8 +102,11 @@ int ig_run_finalize(ig_ctx* c, int channel, float* image, double* norm_host, boo
     int launches = 0;
     dim3 g((N + 255) / 256, N), b(256);
     // Stokes parameter s = sum_p M[s][p] D_p with D_p = img_p / N_p (reading 21); the coefficients carry N_ref / N_p so that
-    // the grids keep their scale through the fp32 FFT and k_fin_write divides by N_ref = N_0 in fp64
-    const double nref = acc.norm[0];
+    // the grids keep their scale through the fp32 FFT and k_fin_write divides by N_ref in fp64. N_ref is the largest
+    // normaliser in magnitude, so a fully flagged polarisation (N_p = 0, and then an all-zero grid) cannot zero the
+    // scale of the others; such a polarisation enters the combinations as D_p = 0 (reading 21)
+    double nref = 0.0;
+    for (int p = 0; p < npol; ++p) if (fabs(acc.norm[p]) > fabs(nref)) nref = acc.norm[p];
     for (int q = 0; q < npol; ++q) {
         if (stokes && npol > 1) {
             double m[4][2] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}};          // complex coefficient per polarisation

@@ -286,3 +286,15 @@ def test_stokes_conversion_recovers_a_polarised_source(orc, npol):
     # the plain finaliser's images are the correlations themselves: XX = I + Q, YY = I - Q (real parts)
     plain = orc.finalize(g, nrm, beta)[:, b0 + n // 2, a0 + n // 2]
     assert np.abs(plain - np.real(corr)).max() < 5e-3
+    if npol == 4:
+        # XX flagged throughout (weight 0: N_XX = 0, grid plane zero): it enters as D_XX = 0 (reading 21), so U and V, which
+        # need only XY and YX, are unchanged to the last bit, I = D_YY / 2 = (I - Q)/2, Q = -(I - Q)/2, nothing is NaN
+        wt0 = wt.copy()
+        wt0[..., 0] = 0.0
+        g0, nrm0, _ = orc.grid_records(idx, vis, wt0, n, beta, [S], bank, off)
+        assert nrm0[0] == 0.0 and not np.any(g0[..., 0])
+        st0 = orc.finalize_stokes(g0, nrm0, beta)
+        assert np.isfinite(st0).all()
+        assert np.array_equal(st0[2:], st[2:])
+        got0 = st0[:, b0 + n // 2, a0 + n // 2]
+        assert abs(got0[0] - (I - Q) / 2) < 5e-3 and abs(got0[1] + (I - Q) / 2) < 5e-3
