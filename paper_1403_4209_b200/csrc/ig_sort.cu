@@ -8,8 +8,8 @@
 // -> stable scatter. Stability keeps the input (time) order inside a (tile, baseline) run.
 // The tile part is new: rows whose footprints fall in the same 2-D region of the grid are
 // made neighbours in the work queue, so that the pixel commits of concurrently running
-// warps meet in the L2 instead of each costing an HBM read and write-back (profiles/
-// r01_v0_gridder.md: 1.0 TB of DRAM traffic on config 5 for 24 M touched pixels). A track
+// warps meet in the L2 instead of each costing an HBM read and write-back (round 1's first gridder, without
+// the tile key: 1.0 TB of DRAM traffic on config 5 for 24 M touched pixels). A track
 // that crosses a tile edge is cut there, which costs one flush of the lane registers.
 // Output: perm[j] = input row at sorted place j.
 #include "ig_internal.h"
@@ -142,16 +142,49 @@ __device__ __forceinline__ uint32_t spread8(uint32_t x) {
     x = (x | (x << 1)) & 0x5555u;
     return x;
 }
-__global__ void k_sort_keys(const double* __restrict__ uvw, const int* __restrict__ baseline_id, long long n,
-                            double cells_per_m, int N, int tile_shift, uint64_t* __restrict__ keys) {
-    long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (r >= n) return;
+__device__ __forceinline__ uint64_t row_key(const double* __restrict__ uvw, const int* __restrict__ baseline_id, long long r,
+                                           double cells_per_m, int N, int tile_shift) {
     double u = uvw[3 * r], v = uvw[3 * r + 1], w = uvw[3 * r + 2];
     if (w < 0.0) { u = -u; v = -v; }
     double fx = u * cells_per_m + 0.5 * N, fy = v * cells_per_m + 0.5 * N;
     int x = (int)fmin(fmax(fx, 0.0), (double)(N - 1)), y = (int)fmin(fmax(fy, 0.0), (double)(N - 1));
     uint32_t m = spread8((uint32_t)(x >> tile_shift)) | (spread8((uint32_t)(y >> tile_shift)) << 1);
-    keys[r] = ((uint64_t)m << 32) | (uint32_t)baseline_id[r];
+    return ((uint64_t)m << 32) | (uint32_t)baseline_id[r];
+}
+__global__ void k_sort_keys(const double* __restrict__ uvw, const int* __restrict__ baseline_id, long long n,
+                            double cells_per_m, int N, int tile_shift, uint64_t* __restrict__ keys) {
+    long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n) return;
+    keys[r] = row_key(uvw, baseline_id, r, cells_per_m, N, tile_shift);
+}
+
+// Small batches (n <= SORT_SMALL_MAX rows: a chunk fed by a streaming caller; configuration 1's 1 792
+// rows): the 25 launches of the radix sort cost more than the whole gridding (PAPER.md:2008 makes the same remark
+// about preparation on the light configuration). One CTA instead: key and input place are packed into one 64-bit
+// word, (48-bit key) << 12 | row, which makes every word distinct, so a plain bitonic network in shared memory
+// yields exactly the stable order of the radix sort (ties broken by input place) and needs no scratch.
+#define SORT_SMALL_MAX 4096
+__global__ void __launch_bounds__(1024)
+k_sort_small(const double* __restrict__ uvw, const int* __restrict__ baseline_id, int n, double cells_per_m, int N,
+             int tile_shift, uint32_t* __restrict__ perm_out) {
+    __shared__ uint64_t s[SORT_SMALL_MAX];
+    int np2 = 32;
+    while (np2 < n) np2 <<= 1;
+    for (int i = threadIdx.x; i < np2; i += blockDim.x)
+        s[i] = i < n ? ((row_key(uvw, baseline_id, i, cells_per_m, N, tile_shift) << 12) | (uint64_t)i) : ~0ull;
+    __syncthreads();
+    for (int k = 2; k <= np2; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int t = threadIdx.x; t < (np2 >> 1); t += blockDim.x) {
+                const int i = 2 * j * (t / j) + (t % j), l = i + j;      // pair t of this stage: places i < l, j apart
+                const bool ascending = (i & k) == 0;
+                const uint64_t a = s[i], b = s[l];
+                if ((a > b) == ascending) { s[i] = b; s[l] = a; }
+            }
+            __syncthreads();
+        }
+    }
+    for (int i = threadIdx.x; i < n; i += blockDim.x) perm_out[i] = (uint32_t)(s[i] & (SORT_SMALL_MAX - 1));
 }
 
 size_t ig_sort_scratch_bytes(long long nrow) {
@@ -181,6 +214,11 @@ int ig_launch_sort_rows(ig_ctx* c, const double* uvw, const int* baseline_id, lo
     while ((c->prm.N >> tile_shift) > 8) ++tile_shift;
     if (c->tile_shift) tile_shift = c->tile_shift;      // ig_set_sort_tile_shift
     const double cells_per_m = ref_freq_hz * c->prm.ku / (double)c->prm.beta;
+    if (nrow <= SORT_SMALL_MAX) {
+        k_sort_small<<<1, 1024, 0, c->stream>>>(uvw, baseline_id, (int)nrow, cells_per_m, c->prm.N, tile_shift, perm_out);
+        IG_CUDA_OK(c, cudaGetLastError());
+        return 1;
+    }
     k_sort_keys<<<(unsigned)((nrow + 255) / 256), 256, 0, c->stream>>>(uvw, baseline_id, nrow, cells_per_m, c->prm.N,
                                                                       tile_shift, keysA);
     int launches = 1;
