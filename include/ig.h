@@ -62,7 +62,12 @@ const char* ig_last_error(const ig_ctx* ctx);
  * with pol = 2*pair + k, so that a pixel commit is two 16-byte vector reductions and neighbouring
  * pixels share L2 sectors. Pixel (N/2,N/2) is u=v=0. */
 size_t ig_grid_bytes(const ig_ctx* ctx);
-/* Bytes of work_dev that one ig_grid call of (nrow, nchan) needs. */
+/* Bytes of work_dev that one ig_grid call of (nrow, nchan) needs, for the context as it stands: the plan arrays and
+ * the entry area of the gather gridder (80 B per record at 4 polarisations, the largest part) are counted only when a
+ * record can reach it, i.e. not when the installed support table stays below ig_set_gather_min_support's threshold
+ * (before a table is installed, max_support decides); with per-channel grids the plan arrays grow with nchan. Ask again
+ * after changing the table, the threshold or the per-channel switch; ig_grid checks the bound size and returns
+ * IG_ENOMEM if short. */
 size_t ig_workspace_bytes(const ig_ctx* ctx, long long nrow, int nchan);
 /* Bytes of the kernel bank for this support table [n_wplanes] (host; NULL = upper
  * bound with every plane at max_support). */
@@ -176,7 +181,7 @@ ig_status ig_set_stokes_output(ig_ctx* ctx, int on);
  * (registers follow a track, atomics when a pixel leaves the window, :710-742); records with support >= s go to
  * the fixed-tile gather gridder (a warp owns an 8 x 16 pixel tile in registers, records binned by tile, no atomics
  * in the loop). Default 25 (measured crossover on configurations 3-5). s = 1: everything through the gather gridder; s > IG_MAX_SUPPORT: nothing. Same grid
- * up to fp32 summation order. Per-channel grids always use the moving window. */
+ * up to fp32 summation order. */
 ig_status ig_set_gather_min_support(ig_ctx* ctx, int s);
 
 /* Ordering (A2): rows are sorted by (uv tile in Morton order, baseline, time). shift = log2 of the tile side in
@@ -185,7 +190,9 @@ ig_status ig_set_sort_tile_shift(ig_ctx* ctx, int shift);
 
 /* One grid per channel (the thesis's default mode, :1011, :1120; reading 16): with the switch on, grid_dev holds nchan
  * grids back to back (each ig_grid_bytes(), same layout), channel c of every ig_grid call goes to grid c with its own
- * normaliser, and ig_finalize_channel images one of them. Up to 4096 channels. Switch it before the first ig_grid. */
+ * normaliser, and ig_finalize_channel images one of them. Up to 4096 channels. Switch it before the first ig_grid.
+ * Both work distributions serve this mode (the gather gridder's tile plan then covers nchan grids: its bins are
+ * (w-plane bucket, channel, tile), 12 B of workspace each, nchan * 16 * (N/32)^2 of them). */
 ig_status ig_set_per_channel_grids(ig_ctx* ctx, int on);
 ig_status ig_finalize_channel(ig_ctx* ctx, int channel, float* image_dev, double* normaliser_host);
 
@@ -210,7 +217,10 @@ ig_status ig_set_commit_counting(ig_ctx* ctx, int on);
 ig_status ig_measure_fp32_peak(void* cuda_stream, void* sink_dev, double* tflops);
 /* Measured rate of the gridder's commit (one 32-byte 4-pol pixel = 2 x red.global.add.v4.f32) at
  * pseudo-random places of buf_dev (dev, `bytes` long, contents are added to), in 1e9 pixel commits/s.
- * run_len = consecutive pixels committed by neighbouring lanes (1..32). The atomic ceiling of the
+ * |run_len| = consecutive pixels committed by neighbouring lanes (1..32). The SIGN of run_len picks the pixel layout:
+ * run_len > 0: the two 16-byte halves of a pixel are neighbours (pixel-interleaved, 32 B per pixel); run_len < 0: the
+ * gridder's own 4-pol layout, two planes of polarisation pairs (ig_grid_bytes above), which is the ceiling that
+ * applies to ig_grid (bench.py passes -8). 0 or |run_len| > 32: IG_EINVAL. The atomic ceiling of the
  * roofline: L2-resident when bytes << 126 MB, HBM-backed when bytes >> 126 MB. */
 ig_status ig_measure_commit_rate(void* cuda_stream, void* buf_dev, size_t bytes, int run_len,
                                  double* gcommits_per_s);

@@ -36,16 +36,19 @@ GridLayout grid_layout(const ig_ctx* c, long long nrow, int nchan) {
     L.sort = o; o += ig_align(ig_sort_scratch_bytes(nrow));
     L.smax = o; o += ig_align((size_t)L.n_chunks * 4);
     L.gcount = o; o += ig_align((size_t)L.n_chunks * 4);          // directly after smax (cleared together)
-    const size_t nt = ig_gather_bins(c);
+    // the gather gridder's plan arrays and entry area exist only when a record can reach it (ig_gather_possible):
+    // support tables below the threshold need none of them
+    const bool gather = ig_gather_possible(c);
+    const size_t nt = gather ? ig_gather_bins(c, nchan) : 0;
     L.tile_count = o; o += ig_align(nt * 4);
     L.tile_off = o; o += ig_align(nt * 4);
     L.tile_cur = o; o += ig_align(nt * 4);
     L.plan_hdr = o; o += 256;
-    L.plan_scratch = o; o += ig_align(ig_gather_plan_scratch_bytes(c));
-    L.items = o; o += ig_align(ig_gather_max_items(c, L.n_chunks) * 16);
+    L.plan_scratch = o; o += gather ? ig_align(ig_gather_plan_scratch_bytes(c, nchan)) : 0;
+    L.items = o; o += gather ? ig_align(ig_gather_max_items(c, L.n_chunks, nchan) * 16) : 0;
     const size_t rec_bytes = ig_align((size_t)L.n_chunks * IG_CH * ig_rec_stride(c->prm.npol));
     L.records = o; o += rec_bytes;
-    L.entries = o; o += ig_align((size_t)L.n_chunks * IG_CH * (16 + 16 * c->prm.npol));   // gather entries: at most every record
+    L.entries = o; o += gather ? ig_align((size_t)L.n_chunks * IG_CH * (16 + 16 * c->prm.npol)) : 0;   // gather entries: at most every record
     L.total = o;
     return L;
 }
@@ -262,8 +265,8 @@ ig_status ig_grid(ig_ctx* c, const double* uvw, const int* baseline_id, long lon
     c->launches += n;
     uint32_t* gcount = (uint32_t*)(c->work + L.gcount);
     uint32_t* tile_count = (uint32_t*)(c->work + L.tile_count);
-    // per-channel grids keep every record with the moving-window gridder (the tile plan is per grid)
-    const int gather_min = c->per_channel ? (IG_MAX_SUPPORT + 1) : c->gather_min;
+    const bool any_gather = ig_gather_possible(c);
+    const int gather_min = any_gather ? c->gather_min : (IG_MAX_SUPPORT + 1);
     n = ig_launch_index(c, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, smax, gcount, tile_count, gather_min);
     if (n < 0) return IG_ECUDA;
     c->launches += n;
@@ -272,10 +275,8 @@ ig_status ig_grid(ig_ctx* c, const double* uvw, const int* baseline_id, long lon
     if (n < 0) return IG_ECUDA;
     c->launches += n;
     cudaEventRecord(ev[2], c->stream);
-    bool any_gather = false;
-    for (int p = 0; p < c->prm.P; ++p) any_gather |= c->support[p] >= gather_min;
     if (any_gather) {
-        n = ig_launch_gather(c, records, gcount, L.n_chunks, tile_count, (uint32_t*)(c->work + L.tile_off),
+        n = ig_launch_gather(c, records, gcount, L.n_chunks, nchan, tile_count, (uint32_t*)(c->work + L.tile_off),
                              (uint32_t*)(c->work + L.tile_cur), (uint4*)(c->work + L.items), (uint32_t*)(c->work + L.plan_hdr),
                              c->work + L.entries, (unsigned long long*)(c->work + L.plan_scratch));
         if (n < 0) return IG_ECUDA;

@@ -18,9 +18,11 @@
 // Plan (the thesis's scan / compaction / plan steps, Alg 4.2-4.3 :1446-1508, rebuilt for this ownership):
 //   k_index            marks large-support records (IG_HDR_GATHER) and counts them per 32 x 32 "origin tile"
 //                      (the tile that holds the footprint's first pixel)
-//   k_gather_plan      one CTA: exclusive scan of the counts -> tile offsets; cuts every tile's list into items
-//                      of <= IG_GCH records
-//   k_gather_scatter   counting-sort scatter of the marked records into tile order (header rewritten relative
+//                      and w-plane bucket: bin = bucket * tiles + tile, bucket-major, so that the kernel matrices
+//                      in use at any time stay in L2
+//   k_gather_plan_a/b/c  multi-CTA exclusive scan of the bin counts (per-block sums, one CTA over the block sums,
+//                      per-block scan with carry) -> bin offsets; cuts every bin's list into items of <= IG_GCH records
+//   k_gather_scatter   counting-sort scatter of the marked records into bin order (header rewritten relative
 //                      to the tile)
 //   k_gather           persistent CTAs; an item's records are staged once into shared memory by the TMA bulk-copy
 //                      engine; the CTA's warps take the 8 x 16 sub-tiles of the region the item can reach
@@ -158,7 +160,7 @@ __global__ void __launch_bounds__(1024) k_gather_plan_c(const uint32_t* __restri
 template <int NPOL>
 __global__ void __launch_bounds__(256) k_gather_scatter(const char* __restrict__ records, const uint32_t* __restrict__ gcount,
                                                         long long n_chunks, uint32_t* __restrict__ tile_cur, int tiles_x,
-                                                        uint32_t ntiles, int n_planes, char* __restrict__ entries) {
+                                                        uint32_t ntiles, int n_planes, char* __restrict__ entries, int nchan_grids) {
     constexpr int STRIDE = NPOL == 4 ? 48 : 32;
     constexpr int GSTRIDE = 16 + 16 * NPOL;
     const long long chunk = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
@@ -172,8 +174,11 @@ __global__ void __launch_bounds__(256) k_gather_scatter(const char* __restrict__
         if (!gm) continue;
         if (mine) {
             const int X0 = (int)(h.x & 0xffffu), Y0 = (int)(h.x >> 16);
-            const uint32_t tile = ig_gather_bin((int)(h.z & IG_HDR_GPLANE), n_planes, ntiles,
-                                                (uint32_t)((Y0 >> IG_GT_SHIFT) * tiles_x + (X0 >> IG_GT_SHIFT)));
+            // per-channel grids (nchan_grids > 0): the channel of this work item selects the grid, tile = channel * tiles + tile
+            const uint32_t tl = (uint32_t)((Y0 >> IG_GT_SHIFT) * tiles_x + (X0 >> IG_GT_SHIFT));
+            const uint32_t tile = nchan_grids > 0
+                ? ig_gather_bin((int)(h.z & IG_HDR_GPLANE), n_planes, ntiles * (uint32_t)nchan_grids, (uint32_t)(chunk % nchan_grids) * ntiles + tl)
+                : ig_gather_bin((int)(h.z & IG_HDR_GPLANE), n_planes, ntiles, tl);
             const uint32_t peers = __match_any_sync(gm, tile);
             const int leader = __ffs(peers) - 1;
             uint32_t base = 0;
@@ -299,11 +304,11 @@ struct GScan {
     }
 };
 
-template <int NPOL, bool COUNT>
+template <int NPOL, bool COUNT, bool PERCH>
 __global__ void __launch_bounds__(IG_GW * 32, IG_GCTAS_PER_SM)
 k_gather(const char* __restrict__ entries, const uint4* __restrict__ items, const uint32_t* __restrict__ plan_hdr,
          float* __restrict__ grid, const float2* __restrict__ bank, int N, int tiles_x, uint32_t ntiles, unsigned* __restrict__ ticket,
-         unsigned long long* __restrict__ commits) {
+         unsigned long long* __restrict__ commits, uint32_t ntiles_v) {
     constexpr int GSTRIDE = 16 + 16 * NPOL;
     __shared__ __align__(128) char buf[IG_GCH * GSTRIDE];
     __shared__ __align__(8) uint64_t bar;
@@ -347,7 +352,17 @@ k_gather(const char* __restrict__ entries, const uint4* __restrict__ items, cons
         smax = __reduce_max_sync(0xffffffffu, smax);
         const int nsx = (IG_GT - 1 + smax + 7) >> 3, nsy = (IG_GT - 1 + smax + 4 * IG_GR - 1) / (4 * IG_GR);
         const unsigned nsub = (unsigned)(nsx * nsy);
-        const int tile_id = (int)(item.x % ntiles);        // item.x = plane bucket * ntiles + origin tile
+        // item.x = plane bucket * ntiles_v + channel * ntiles + origin tile (one grid: ntiles_v = ntiles, channel = 0)
+        // PERCH (per-channel grids, back to back in memory): grid ch is reached by a row offset, since in every layout
+        // ([N][N][npol]; 4 pol: [2][N][N][2]) a whole grid is N (2N for 4 pol) rows of N pixels at the stride pix is scaled by
+        int tile_id, row0 = 0;
+        if constexpr (PERCH) {
+            const uint32_t tile_v = item.x % ntiles_v, ch = tile_v / ntiles;
+            tile_id = (int)(tile_v - ch * ntiles);
+            row0 = (int)ch * N * (NPOL == 4 ? 2 : 1);
+        } else {
+            tile_id = (int)(item.x % ntiles);
+        }
         const int tile_y = tile_id / tiles_x, tile_x = tile_id - tile_y * tiles_x;
         for (;;) {
             unsigned st = 0;
@@ -398,7 +413,7 @@ k_gather(const char* __restrict__ entries, const uint4* __restrict__ items, cons
 #pragma unroll
                 for (int q = 0; q < NPOL; ++q) any |= __float_as_uint(acc[k][q].x) | __float_as_uint(acc[k][q].y);
                 if ((any << 1) != 0u && x < N && y < N) {          // some sum is not +-0
-                    const size_t pix = (size_t)y * N + x;
+                    const size_t pix = (size_t)(row0 + y) * N + x;
                     float a[2 * NPOL];
 #pragma unroll
                     for (int q = 0; q < NPOL; ++q) { a[2 * q] = acc[k][q].x; a[2 * q + 1] = acc[k][q].y; }
@@ -428,18 +443,21 @@ size_t ig_gather_tiles(const ig_ctx* c) {
     const size_t t = (size_t)((c->prm.N + IG_GT - 1) / IG_GT);
     return t * t;
 }
-size_t ig_gather_bins(const ig_ctx* c) { return ig_gather_tiles(c) * IG_GBUCKETS; }
-size_t ig_gather_max_items(const ig_ctx* c, long long n_chunks) {
-    return (size_t)n_chunks * IG_CH / IG_GCH + ig_gather_bins(c) + 1;
+size_t ig_gather_bins(const ig_ctx* c, int nchan) { return ig_gather_tiles(c) * (c->per_channel ? (size_t)nchan : 1) * IG_GBUCKETS; }
+size_t ig_gather_max_items(const ig_ctx* c, long long n_chunks, int nchan) {
+    return (size_t)n_chunks * IG_CH / IG_GCH + ig_gather_bins(c, nchan) + 1;
 }
-size_t ig_gather_plan_scratch_bytes(const ig_ctx* c) { return ((ig_gather_bins(c) + 4095) / 4096) * 8; }
+size_t ig_gather_plan_scratch_bytes(const ig_ctx* c, int nchan) { return ((ig_gather_bins(c, nchan) + 4095) / 4096) * 8; }
 
-int ig_launch_gather(ig_ctx* c, const char* records, const uint32_t* gcount, long long n_chunks, uint32_t* tile_count,
+int ig_launch_gather(ig_ctx* c, const char* records, const uint32_t* gcount, long long n_chunks, int nchan, uint32_t* tile_count,
                      uint32_t* tile_off, uint32_t* tile_cur, uint4* items, uint32_t* plan_hdr, char* entries,
                      unsigned long long* plan_scratch) {
     if (n_chunks == 0) return 0;
     cudaStream_t stream = c->stream;
-    const uint32_t ntiles = (uint32_t)ig_gather_tiles(c), nbins = (uint32_t)ig_gather_bins(c);
+    if (ig_gather_bins(c, nchan) >= (1ull << 32)) { c->err = "gather plan: too many (channel, tile) bins"; return -1; }
+    const uint32_t ntiles = (uint32_t)ig_gather_tiles(c), nbins = (uint32_t)ig_gather_bins(c, nchan);
+    const int nchan_grids = c->per_channel ? nchan : 0;
+    const uint32_t ntiles_v = ntiles * (uint32_t)(c->per_channel ? nchan : 1);
     const int tiles_x = (c->prm.N + IG_GT - 1) / IG_GT;
     const uint32_t nblocks = (nbins + 4095u) / 4096u;
     k_gather_plan_a<<<nblocks, 1024, 0, stream>>>(tile_count, plan_scratch, nbins);
@@ -447,21 +465,24 @@ int ig_launch_gather(ig_ctx* c, const char* records, const uint32_t* gcount, lon
     k_gather_plan_c<<<nblocks, 1024, 0, stream>>>(tile_count, plan_scratch, tile_off, tile_cur, items, nbins);
     const unsigned sblocks = (unsigned)((n_chunks + 7) / 8);
     switch (c->prm.npol) {
-        case 1: k_gather_scatter<1><<<sblocks, 256, 0, stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, ntiles, c->prm.P, entries); break;
-        case 2: k_gather_scatter<2><<<sblocks, 256, 0, stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, ntiles, c->prm.P, entries); break;
-        default: k_gather_scatter<4><<<sblocks, 256, 0, stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, ntiles, c->prm.P, entries); break;
+        case 1: k_gather_scatter<1><<<sblocks, 256, 0, stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, ntiles, c->prm.P, entries, nchan_grids); break;
+        case 2: k_gather_scatter<2><<<sblocks, 256, 0, stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, ntiles, c->prm.P, entries, nchan_grids); break;
+        default: k_gather_scatter<4><<<sblocks, 256, 0, stream>>>(records, gcount, n_chunks, tile_cur, tiles_x, ntiles, c->prm.P, entries, nchan_grids); break;
     }
     IG_CUDA_OK(c, cudaMemsetAsync(&c->d_acc->ticket_gather, 0, sizeof(unsigned), stream));
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     dim3 g((unsigned)(sms * IG_GCTAS_PER_SM)), b(IG_GW * 32);
-#define IG_GLAUNCH(P, C) k_gather<P, C><<<g, b, 0, stream>>>(entries, items, plan_hdr, c->grid, c->d_bank, c->prm.N, tiles_x, ntiles, &c->d_acc->ticket_gather, &c->d_acc->commits)
+#define IG_GLAUNCH2(P, C, G) k_gather<P, C, G><<<g, b, 0, stream>>>(entries, items, plan_hdr, c->grid, c->d_bank, c->prm.N, tiles_x, ntiles, &c->d_acc->ticket_gather, &c->d_acc->commits, ntiles_v)
+#define IG_GLAUNCH(P, C) do { if (c->per_channel) IG_GLAUNCH2(P, C, true); else IG_GLAUNCH2(P, C, false); } while (0)
+    if ((long long)c->prm.N * (c->prm.npol == 4 ? 2 : 1) * (c->per_channel ? nchan : 1) >= (1ll << 31)) { c->err = "per-channel grids: too many grid rows for the gather gridder"; return -1; }
     if (c->count_commits) {
         switch (c->prm.npol) { case 1: IG_GLAUNCH(1, true); break; case 2: IG_GLAUNCH(2, true); break; default: IG_GLAUNCH(4, true); break; }
     } else {
         switch (c->prm.npol) { case 1: IG_GLAUNCH(1, false); break; case 2: IG_GLAUNCH(2, false); break; default: IG_GLAUNCH(4, false); break; }
     }
+#undef IG_GLAUNCH2
 #undef IG_GLAUNCH
     IG_CUDA_OK(c, cudaGetLastError());
     return 5;

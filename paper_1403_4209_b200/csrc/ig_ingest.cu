@@ -188,7 +188,10 @@ k_index(IgParams P, const IgPlaneEntry* __restrict__ planes, const double* __res
                     hdr.z = IG_HDR_GATHER | (conj ? IG_HDR_CONJ : 0u) | pstore;
                     hdr.w = (uint32_t)S;
                     // plan bin: (w-plane bucket, origin tile of 32 x 32 pixels)
-                    g_tile = ig_gather_bin((int)pstore, P.P, (uint32_t)(tiles_x * tiles_x), (uint32_t)((b0 >> 5) * tiles_x + (a0 >> 5)));
+                    // per-channel grids: the channel selects the grid, tile = channel * tiles + tile (as k_gather_scatter)
+                    const uint32_t nt = (uint32_t)(tiles_x * tiles_x), tl = (uint32_t)((b0 >> 5) * tiles_x + (a0 >> 5));
+                    g_tile = chan_norm ? ig_gather_bin((int)pstore, P.P, nt * (uint32_t)nchan, (uint32_t)c * nt + tl)
+                                       : ig_gather_bin((int)pstore, P.P, nt, tl);
                 } else {
                     hdr.x = (uint32_t)(b0 * P.N + a0);
                     hdr.z = IG_HDR_PACK(cm, dm, S) | (conj ? IG_HDR_CONJ : 0u);
@@ -323,7 +326,8 @@ int ig_launch_index(ig_ctx* c, const double* uvw, const uint32_t* perm, long lon
     if (nrb > 0x7fffffffll) { c->err = "too many rows"; return -1; }
     // chunk_smax and gcount are neighbours in the work buffer: one memset clears both
     IG_CUDA_OK(c, cudaMemsetAsync(chunk_smax, 0, (size_t)((char*)(gcount + nrb * nchan) - (char*)chunk_smax), c->stream));
-    IG_CUDA_OK(c, cudaMemsetAsync(tile_count, 0, ig_gather_bins(c) * 4, c->stream));
+    if (gather_min <= IG_MAX_SUPPORT)   // the plan's bin counts exist only when a record can reach the gather gridder (grid_layout)
+        IG_CUDA_OK(c, cudaMemsetAsync(tile_count, 0, ig_gather_bins(c, nchan) * 4, c->stream));
     dim3 g((unsigned)nrb), b(IG_CH);
     const int tiles_x = (c->prm.N + 31) / 32;
 #define IG_INDEX(P_) k_index<P_><<<g, b, 0, c->stream>>>(c->prm, c->d_planes, c->d_zeta, uvw, perm, nrow, d_freqs, nchan, vis, wt, records, chunk_smax, c->d_acc, c->compress, c->per_channel ? c->d_chan_norm : nullptr, gcount, tile_count, gather_min, tiles_x)

@@ -88,6 +88,14 @@ struct ig_ctx {
     std::string err;
 };
 
+// Can any record of an ig_grid call go to the gather gridder? Not when no plane's support reaches the threshold.
+// Before a support table is installed the answer is the cautious one. Decides whether the plan arrays and the entry
+// area of the workspace exist at all.
+static inline bool ig_gather_possible(const ig_ctx* c) {
+    if (c->support.empty()) return c->max_support >= c->gather_min;
+    for (int s : c->support) if (s >= c->gather_min) return true;
+    return false;
+}
 static inline size_t ig_align(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 static inline int ig_rec_stride(int npol) { return npol == 4 ? 48 : 32; }  // bytes, multiple of 16
 
@@ -103,15 +111,16 @@ int ig_launch_index(ig_ctx* c, const double* uvw, const uint32_t* perm, long lon
                     const double* d_freqs, int nchan, const float* vis, const float* wt,
                     char* records, uint32_t* chunk_smax, uint32_t* gcount, uint32_t* tile_count, int gather_min);   // uses c->per_channel / c->d_chan_norm
 // gather gridder (ig_gather.cu): plan, scatter, gridder; gcount[chunk] = marked records per work item
+// With per-channel grids (c->per_channel) the plan covers nchan grids: the "tile" of a bin is then channel * tiles + tile.
 size_t ig_gather_tiles(const ig_ctx* c);
-size_t ig_gather_bins(const ig_ctx* c);
-size_t ig_gather_plan_scratch_bytes(const ig_ctx* c);
+size_t ig_gather_bins(const ig_ctx* c, int nchan);
+size_t ig_gather_plan_scratch_bytes(const ig_ctx* c, int nchan);
 // plan bin of a gather record (both k_index and k_gather_scatter call it)
 __host__ __device__ static inline uint32_t ig_gather_bin(int plane, int n_planes, uint32_t ntiles, uint32_t tile) {
     return (uint32_t)(((long long)plane * IG_GBUCKETS) / n_planes) * ntiles + tile;
 }
-size_t ig_gather_max_items(const ig_ctx* c, long long n_chunks);
-int ig_launch_gather(ig_ctx* c, const char* records, const uint32_t* gcount, long long n_chunks, uint32_t* tile_count,
+size_t ig_gather_max_items(const ig_ctx* c, long long n_chunks, int nchan);
+int ig_launch_gather(ig_ctx* c, const char* records, const uint32_t* gcount, long long n_chunks, int nchan, uint32_t* tile_count,
                      uint32_t* tile_off, uint32_t* tile_cur, uint4* items, uint32_t* plan_hdr, char* entries,
                      unsigned long long* plan_scratch);
 int ig_launch_debug_index(ig_ctx* c, const double* uvw, long long nrow, const double* d_freqs, int nchan,

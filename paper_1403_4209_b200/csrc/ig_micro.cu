@@ -91,7 +91,7 @@ __global__ void __launch_bounds__(256) k_red_rate(float* buf, unsigned long long
 
 extern "C" ig_status ig_measure_commit_rate(void* cuda_stream, void* buf_dev, size_t bytes, int run_len,
                                             double* gcommits_per_s) {
-    const int planar = run_len < 0;          // negative run length: planar polarisation-pair layout (experiment)
+    const int planar = run_len < 0;          // negative run length: the gridder's planar polarisation-pair layout (documented in include/ig.h)
     if (planar) run_len = -run_len;
     if (!buf_dev || bytes < 4096 || !gcommits_per_s || run_len < 1 || run_len > 32) return IG_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;

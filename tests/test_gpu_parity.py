@@ -162,6 +162,28 @@ def test_grid_matches_oracle_own_bank(name, runs, torch_cuda):
     assert g.last_launches() > 0
 
 
+@pytest.mark.parametrize("name", ["cfg3s", "cfg5s"])
+def test_grid_matches_oracle_support_law_k(name, orc, torch_cuda):
+    """The alternative support law of reading 8 (support linear in the plane index instead of in |w|; SURVEY 8(c):
+    both laws reported): it moves several times more of the updates into supports at and above the gather threshold,
+    so it is the harder case for the fixed-tile gridder. Own bank, default work distribution."""
+    wl = synth.make_workload(CASES[name], support_law="k")
+    wl_w = synth.make_workload(CASES[name], with_vis=False)
+    big = lambda sup: int((sup.astype(np.int64)[sup >= 25] ** 2).sum())
+    assert big(wl["supports"]) > 1.5 * big(wl_w["supports"])
+    ref = oracle_run(orc, wl)
+    g = make_gridder(wl)
+    g.build_wkernels(wl["w_max"])
+    uvw, bl, vis, wt = to_dev(torch_cuda, wl)
+    g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+    check_grid(g.grid_complex(), ref["grid"])
+    assert g.stats() == tuple(int(x) for x in ref["stats"])
+    window_ms, gather_ms = g.gridder_split()
+    assert gather_ms > 0
+    _, norm = g.finalize()
+    assert np.allclose(norm, ref["norm"], rtol=1e-6, atol=0)
+
+
 @pytest.mark.parametrize("name", ["cfg2s", "cfg5s"])
 def test_grid_matches_oracle_injected_bank(name, runs, torch_cuda):
     """Isolates the gridder: both sides use the oracle's bank (rounded to complex64 for the GPU)."""
@@ -427,7 +449,6 @@ def test_compression_same_grid_and_counts(orc, torch_cuda):
 
 
 WINDOW = 512          # side of the full-size parity windows (pixels)
-PARITY_LOG = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out", "fullsize_parity.jsonl")
 
 
 def _full_size_window_check(orc, torch_cuda, cfg_index, n_pixels=0, seed=0):
@@ -495,13 +516,7 @@ def _full_size_window_check(orc, torch_cuda, cfg_index, n_pixels=0, seed=0):
                "planes": int(planes.size), "updates": int(st[2]), "rel_frobenius": frob, "max_over_max": mx,
                "bars": [FROB_TOL, MAX_TOL]}
         out.append(rec)
-        try:
-            os.makedirs(os.path.dirname(PARITY_LOG), exist_ok=True)
-            with open(PARITY_LOG, "a") as f:
-                f.write(json.dumps(rec) + "\n")
-        except OSError:
-            pass
-        print(json.dumps(rec))
+        print("FULLSIZE_PARITY " + json.dumps(rec))     # pytest -rP shows it; the round's table is kept under profiles/
         assert frob <= FROB_TOL, rec
         assert mx <= MAX_TOL, rec
 
@@ -561,19 +576,27 @@ def test_automatic_supports_match_oracle_and_grid(orc, torch_cuda):
     assert g.stats() == tuple(int(x) for x in ref["stats"])
 
 
-def test_per_channel_grids(orc, torch_cuda):
+@pytest.mark.parametrize("npol,s_max,threshold", [(4, 33, None), (4, 33, 1000), (2, 65, None), (1, 21, 1)])
+def test_per_channel_grids(npol, s_max, threshold, orc, torch_cuda):
     """One grid per channel (the thesis's default, :1120): channel c of the batch goes to grid c with its own
-    normaliser; each equals the oracle run on that channel alone; ig_finalize_channel images it."""
+    normaliser; each equals the oracle run on that channel alone; ig_finalize_channel images it. Through both work
+    distributions: the default threshold (supports from 25 up go to the gather gridder, whose plan then carries the
+    channel; the thesis ran its heavy configuration, supports to 349, in this mode, :1988), everything through the
+    moving window, everything through the gather gridder."""
     from paper_1403_4209_b200.binding import Gridder, IgError
-    cfg = small(synth.CONFIGS[1], n_station=9, n_time=150, n_chan=3, n_wplanes=8)
+    cfg = small(synth.CONFIGS[1], n_pol=npol, s_max=s_max, n_station=9, n_time=150, n_chan=3, n_wplanes=8)
     wl = synth.make_workload(cfg)
     sup = wl["supports"]
     bank, off = orc.build_bank(sup, wl["w_max"], wl["du"], cfg.oversampling, int(sup.max()))
     g = Gridder(cfg.grid_n, wl["cell_rad"], cfg.n_wplanes, cfg.oversampling, int(sup.max()), cfg.n_pol)
     g.allocate(sup, n_channel_grids=cfg.n_chan)
     g.debug_set_wkernels(wl["w_max"], bank.astype(np.complex64))
+    if threshold is not None:
+        g.set_gather_min_support(threshold)
     uvw, bl, vis, wt = to_dev(torch_cuda, wl)
     g.grid_visibilities(uvw, bl, wl["freqs_hz"], vis, wt)
+    window_ms, gather_ms = g.gridder_split()
+    assert (gather_ms > 0.01) == (threshold != 1000) and window_ms > 0     # five launches against two event records
     with pytest.raises(IgError):
         g.finalize()                                   # the single-grid finaliser refuses in this mode
     total = np.zeros(3, dtype=np.int64)
@@ -706,6 +729,20 @@ def test_stokes_output_matches_oracle(npol, orc, torch_cuda):
     assert np.abs(got[:, b0 + n // 2, a0 + n // 2] - [I, Q, U, V][:npol]).max() < 2e-2
     if npol > 1:        # the switch changed the output: the plain images are the correlations
         assert np.abs(plain.cpu().numpy()[0, b0 + n // 2, a0 + n // 2] - (I + Q)) < 2e-2
+    if npol == 4:
+        # polarisation 0 flagged throughout: N_XX = 0 must not wipe out the other Stokes images (D_XX = 0, reading 21)
+        wt0 = wt.copy()
+        wt0[..., 0] = 0.0
+        gr0, nrm0, _ = orc.grid_records(idx, vis, wt0, n, beta, sup, bank, off)
+        want0 = orc.finalize_stokes(gr0, nrm0, beta)
+        g.reset()
+        g.grid_visibilities(torch_cuda.from_numpy(uvw).to(d), torch_cuda.from_numpy(bl).to(d), np.array([C]),
+                            torch_cuda.from_numpy(vis).to(d), torch_cuda.from_numpy(wt0).to(d))
+        img0, norm0 = g.finalize()
+        got0 = img0.cpu().numpy().astype(np.float64)
+        assert norm0[0] == 0.0 and np.isfinite(got0).all()
+        assert np.abs(got0 - want0)[:, inner, inner].max() <= 2e-4 * np.abs(want0[:, inner, inner]).max()
+        assert np.abs(got0[2:, b0 + n // 2, a0 + n // 2] - [U, V]).max() < 2e-2
 
 
 @pytest.mark.parametrize("name,threshold", [("cfg2s", 1), ("cfg5s", 1), ("cfg5s", 1000), ("cfg4s", 13), ("pol2", 1), ("n300", 1)])
