@@ -359,12 +359,16 @@ class Gridder:
     def touched_pixels(self) -> int:
         """Pixels with a non-zero value in any polarisation (synchronises)."""
         t, n = self.torch, self.grid_n
-        g = self.grid.view(2, n * n, 4) if self.n_pol == 4 else self.grid.view(1, n * n, self.n_pol * 2)
-        hit = t.zeros(n * n, dtype=t.bool, device=self.device)
-        for part in g:
-            for lo in range(0, n * n, 1 << 26):
-                hit[lo:lo + (1 << 26)] |= (part[lo:lo + (1 << 26)] != 0).any(dim=1)
-        return int(hit.sum().item())
+        grids = self.grid if getattr(self, "n_channel_grids", 0) > 0 else [self.grid]     # per-channel mode: summed over the grids
+        total = 0
+        for one in grids:
+            g = one.reshape(2, n * n, 4) if self.n_pol == 4 else one.reshape(1, n * n, self.n_pol * 2)
+            hit = t.zeros(n * n, dtype=t.bool, device=self.device)
+            for part in g:
+                for lo in range(0, n * n, 1 << 26):
+                    hit[lo:lo + (1 << 26)] |= (part[lo:lo + (1 << 26)] != 0).any(dim=1)
+            total += int(hit.sum().item())
+        return total
 
     def close(self):
         if self.ctx:
