@@ -143,7 +143,7 @@ ig_status ig_grid_host(ig_ctx* ctx, const double* uvw_m, const int* baseline_id,
  * inside a latency-bound loop where cudaMalloc / cudaFree would stall the whole device, has nobody to ask.
  * This call is ig_grid with its scratch in an array that is part of the library itself (a file-scope
  * __device__ array in csrc/ig_static.cu): same arguments (eq 4.4, steps A1-A3 and C as above), same result up to
- * fp32 summation order, and neither it nor anything it calls allocates or frees device or host memory.
+ * fp32 summation order; it makes no cudaMalloc / cudaFree call and calls no library routine that allocates device memory.
  *   - Limit: ig_workspace_bytes(ctx, nrow, nchan) <= IG_STATIC_WORK_BYTES (32 MiB; e.g. ~230 000 four-polarisation
  *     records on a 2048^2 grid). A larger batch returns IG_ENOMEM, text in ig_last_error, nothing enqueued: feed
  *     smaller batches (ig_grid* calls add up) or use ig_grid.
